@@ -1,0 +1,127 @@
+/* libdg -- C ABI of the B200 nodal-DG hot path (arxiv 1602.07997, PAPER.md).
+ *
+ * What the library computes (everything on one CUDA device, fp32):
+ *   r_k(q)   the semi-discrete right-hand side of PAPER.md eq. (2)-(3):
+ *            volume term   sum_ij g^vol_kij D_j f_jk   (eq. (5)-(6))
+ *            surface term  sum_f g^sur_kf L_f p_kf     with the upwind penalty terms of
+ *            PAPER.md:45-51 (acoustic) and PAPER.md:71-84 (elastic);
+ *   the five-stage fourth-order low-storage Runge-Kutta update named by BASELINE.json
+ *            res <- A_s res + dt r(q),  q <- q + B_s res   (replaces AB3, eq. (4));
+ *   and, as the paper's own integrator, one AB3 step of eq. (4) (dg_ab3_step).
+ *
+ * Conventions:
+ *   reference tetrahedron {r,s,t >= -1, r+s+t <= -1}; local vertices v1=(-1,-1,-1), v2=(1,-1,-1),
+ *   v3=(-1,1,-1), v4=(-1,-1,1) in the order of `etov`; faces f0:(v1,v2,v3) f1:(v1,v2,v4)
+ *   f2:(v2,v3,v4) f3:(v1,v3,v4).  Elements with negative Jacobian have their last two vertices
+ *   swapped at create time (this also swaps which faces the `bc` columns 0/1 and 2/3... refer to:
+ *   `bc` is indexed AFTER the swap, i.e. give positively oriented elements when tags matter).
+ *   Nodes: Np=(N+1)(N+2)(N+3)/6 warp-and-blend nodes in lattice order, t slowest,
+ *   then s, r fastest; dg_node_coords returns their physical coordinates.
+ *   Field layout of q, rhs (DEVICE memory, caller-owned): [K][Nfields][Np] float, node index
+ *   fastest (Table 1).  Acoustic fields (p,vx,vy,vz); elastic fields
+ *   (vx,vy,vz,sxx,syy,szz,sxy,sxz,syz).
+ *
+ * Ownership: host arrays passed to dg_create are only read during the call.  The context owns
+ * all device constants (operators, geometric factors, connectivity) and scratch (residual,
+ * ping-pong state, AB3 history); dg_destroy frees them.  No allocation after dg_create.
+ * dg_rhs/dg_step/dg_run/dg_ab3_step are asynchronous on `cuda_stream` (a cudaStream_t passed as
+ * void*, NULL = default stream) and never synchronise the host.
+ *
+ * Errors: every int function returns 0 on success or a negative DG_ERR_* code; the message is
+ * available from dg_last_error() (thread-local).  No exception crosses the boundary.
+ */
+#ifndef DG_H_
+#define DG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dg_ctx dg_ctx;
+
+enum { DG_ACOUSTIC = 0, DG_ELASTIC = 1 };
+/* tags for faces without a neighbour (reading Q9); SLIP is elastic-only (acoustic: = RIGID) */
+enum { DG_BC_INTERIOR = 0, DG_BC_RIGID = 1, DG_BC_FREE = 2, DG_BC_SLIP = 3 };
+enum {
+  DG_OK = 0,
+  DG_ERR_ARG = -1,      /* NULL pointer, N outside 1..10, unknown model, bad option            */
+  DG_ERR_MESH = -2,     /* non-conforming mesh, degenerate element, untagged boundary face      */
+  DG_ERR_MATERIAL = -3, /* rho<=0, c<=0, vs<=0 or vp <= vs*sqrt(4/3)                            */
+  DG_ERR_CUDA = -4,     /* CUDA runtime failure, or a device entry point on a host-only context */
+  DG_ERR_NOMEM = -5
+};
+
+typedef struct {              /* HOST pointers, borrowed during dg_create                        */
+  int64_t nverts, K;
+  const double *vxyz;         /* [nverts][3]                                                     */
+  const int32_t *etov;        /* [K][4] vertex numbers, any orientation                          */
+  const int8_t *bc;           /* [K][4] DG_BC_* for faces without neighbour; NULL => all RIGID   */
+} dg_mesh;
+
+typedef struct {              /* HOST, per element, fp64 (piecewise-constant media) */
+  const double *rho;          /* [K]                                                             */
+  const double *c_or_vp;      /* [K] acoustic c / elastic c_p                                    */
+  const double *vs;           /* [K] elastic c_s (ignored for acoustic, may be NULL)             */
+} dg_materials;
+
+typedef struct {
+  int device;                 /* CUDA device ordinal; -1 = host-only context (setup introspection,
+                                 no device entry point works: they return DG_ERR_CUDA)           */
+  int variant;                /* 0 = auto; 1 = fused SIMT stage kernel; others reserved          */
+  int elems_per_thread;       /* 0 = auto; register blocking E of the SIMT kernel (1..8)         */
+  int groups_per_cta;         /* 0 = auto; node groups G per CTA (CTA handles G*E elements)      */
+} dg_options;
+
+/* Build a context: reference operators for degree N (1..10), geometric factors, connectivity,
+ * material constants; uploads them and allocates scratch.  `opts` may be NULL (device 0, auto). */
+int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_materials *mat,
+              const dg_options *opts);
+int dg_destroy(dg_ctx *ctx);
+
+/* sizes */
+int dg_num_fields(const dg_ctx *ctx);         /* 4 or 9                                          */
+int dg_np(const dg_ctx *ctx);                 /* nodes per element                               */
+int dg_nfp(const dg_ctx *ctx);                /* nodes per face                                  */
+int64_t dg_num_elements(const dg_ctx *ctx);
+
+/* physical node coordinates, HOST out [K][Np][3] */
+int dg_node_coords(const dg_ctx *ctx, double *xyz_host);
+/* dt = cfl / ((N+1)^2 max_k [c_max,k max_f g^sur_kf])   (reading Q10); <0 on error   */
+double dg_stable_dt(const dg_ctx *ctx, double cfl);
+
+/* r(q) -> d_rhs.  DEVICE pointers, [K][Nfields][Np] float each; d_q is not modified;
+ * d_q == d_rhs is an error.                                                                     */
+int dg_rhs(dg_ctx *ctx, const float *d_q, float *d_rhs, void *cuda_stream);
+/* one LSRK(5,4) step in place on d_q (5 fused stage kernels + one device copy)                  */
+int dg_step(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);
+/* nsteps LSRK steps in place on d_q (5*nsteps fused stage kernels, one copy if that is odd)     */
+int dg_run(dg_ctx *ctx, float *d_q, float dt, int nsteps, void *cuda_stream);
+/* one AB3 step of PAPER.md eq. (4) in place on d_q; the context keeps r^{m-1}, r^{m-2}
+ * (zero after dg_create / dg_ab3_reset, i.e. the first two steps are lower order)               */
+int dg_ab3_step(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);
+int dg_ab3_reset(dg_ctx *ctx, void *cuda_stream);
+
+/* number of kernels/copies the last dg_rhs/dg_step/dg_run/dg_ab3_step call enqueued             */
+int dg_last_launch_count(const dg_ctx *ctx);
+/* name of the kernel variant chosen at create time, e.g. "simt_fused<acoustic,N=5,E=4,G=2>"     */
+const char *dg_variant_name(const dg_ctx *ctx);
+
+/* ---- host-side introspection (no device work; valid on host-only contexts too) -------------
+ * reference operators as the device sees them, fp64 before rounding: Dr,Ds,Dt [Np][Np] row-major,
+ * LIFT [Np][4Nfp] row-major, rst [Np][3], fmask [4][Nfp].  Any pointer may be NULL.             */
+int dg_reference_operators(const dg_ctx *ctx, double *Dr, double *Ds, double *Dt, double *LIFT,
+                           double *rst, int32_t *fmask);
+/* per element geometric factors: G [K][3][3] (G[i][j] = d r_j / d x_i), J [K], nrm [K][4][3],
+ * fscale [K][4]; connectivity as (element, volume node) of the exterior trace of every face
+ * node: elemP, nodeP [K][4Nfp] (boundary faces: the element's own node), bctag [K][4].           */
+int dg_geometry(const dg_ctx *ctx, double *G, double *J, double *nrm, double *fscale);
+int dg_connectivity(const dg_ctx *ctx, int32_t *elemP, int32_t *nodeP, int8_t *bctag);
+
+const char *dg_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DG_H_ */

@@ -35,19 +35,25 @@ class Mesh:
 
 
 def orient(vxyz: np.ndarray, etov: np.ndarray) -> np.ndarray:
-    """Swap the last two vertices of elements with negative Jacobian."""
+    """Swap the last two vertices of elements with negative Jacobian (faces 0 and 1 trade places);
+    returns the new table and the mask of swapped elements."""
     etov = np.array(etov, dtype=np.int64, copy=True)
     v = vxyz[etov]
     det = np.linalg.det(np.stack([v[:, 1] - v[:, 0], v[:, 2] - v[:, 0], v[:, 3] - v[:, 0]], axis=2))
     neg = det < 0
     etov[neg, 2], etov[neg, 3] = etov[neg, 3].copy(), etov[neg, 2].copy()
-    return etov
+    return etov, neg
 
 
 def build(ref: RefElem, vxyz: np.ndarray, etov: np.ndarray, bc: np.ndarray | None = None,
-          chunk: int = 20000) -> Mesh:
+          only_elems: np.ndarray | None = None) -> Mesh:
+    """`only_elems`: restrict the face-node matching (the expensive part) to the faces of these
+    elements; elemP/nodeP rows of all other elements are then left pointing at themselves."""
     vxyz = np.asarray(vxyz, dtype=np.float64)
-    etov = orient(vxyz, etov)
+    etov, swapped = orient(vxyz, etov)
+    if bc is not None:
+        bc = np.array(bc, dtype=np.int8, copy=True)
+        bc[swapped, 0], bc[swapped, 1] = bc[swapped, 1].copy(), bc[swapped, 0].copy()
     K = etov.shape[0]
     Np, Nfp = ref.Np, ref.Nfp
     v = vxyz[etov]                                   # K x 4 x 3
@@ -95,6 +101,11 @@ def build(ref: RefElem, vxyz: np.ndarray, etov: np.ndarray, bc: np.ndarray | Non
     # ---- node matching by physical position on every interior face
     hmin = float(np.min(2.0 / Fscale.max(axis=1)))
     ids = np.flatnonzero(~bnd)
+    if only_elems is not None:
+        keep = np.zeros(K, dtype=bool)
+        keep[np.asarray(only_elems)] = True
+        ids = ids[keep[ids // 4]]
+    chunk = max(256, int(2e7 // (Nfp * Nfp)))
     for c0 in range(0, len(ids), chunk):
         me = ids[c0:c0 + chunk]
         ot = partner[me]

@@ -1,0 +1,455 @@
+// libdg C ABI (include/dg.h): context, host setup -> device upload, kernel dispatch.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <stdexcept>
+#include <string>
+#include <vector>
+
+#include "../../include/dg.h"
+#include "host_setup.hpp"
+#include "kernels.cuh"
+
+// per-(model, degree) kernel getters from stage_inst.cu
+#define DG_DECL(m, n)                                              \
+  extern "C" const void *dgk_get_stage_kernel_##m##_##n(int, int); \
+  extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);
+#define DG_DECL_ALL(m) \
+  DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
+DG_DECL_ALL(0)
+DG_DECL_ALL(1)
+
+namespace {
+typedef const void *(*kernel_getter)(int, int);
+typedef size_t (*smem_getter)(int);
+#define DG_ROW(m, fn)                                                                                          \
+  {nullptr, fn##m##_1, fn##m##_2, fn##m##_3, fn##m##_4, fn##m##_5, fn##m##_6, fn##m##_7, fn##m##_8, fn##m##_9, \
+   fn##m##_10}
+const kernel_getter KERNELS[2][11] = {DG_ROW(0, dgk_get_stage_kernel_), DG_ROW(1, dgk_get_stage_kernel_)};
+const smem_getter SMEM[2][11] = {DG_ROW(0, dgk_stage_smem_bytes_), DG_ROW(1, dgk_stage_smem_bytes_)};
+
+thread_local std::string g_err;
+int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+#define CUDA_TRY(x)                                                                                   \
+  do {                                                                                                \
+    cudaError_t e_ = (x);                                                                             \
+    if (e_ != cudaSuccess) throw std::runtime_error(std::string("cuda: ") + cudaGetErrorString(e_) + " at " #x); \
+  } while (0)
+
+// LSRK(5,4) of Carpenter & Kennedy (BASELINE.json north_star; Q2), exact rationals
+const double RK_A[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
+                        -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+const double RK_B[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
+                        1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
+                        2277821191437.0 / 14882151754819.0};
+}  // namespace
+
+namespace dgk {
+// AB3 update of PAPER.md eq. (4): q += dt (a1 r0 + a2 r1 + a3 r2), pure streaming
+__global__ void ab3_update_kernel(float4 *__restrict__ q, const float4 *__restrict__ r0, const float4 *__restrict__ r1,
+                                  const float4 *__restrict__ r2, size_t n4, float c0, float c1, float c2) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+    float4 a = q[i];
+    const float4 x = r0[i], y = r1[i], z = r2[i];
+    a.x += c0 * x.x + c1 * y.x + c2 * z.x;
+    a.y += c0 * x.y + c1 * y.y + c2 * z.y;
+    a.z += c0 * x.z + c1 * y.z + c2 * z.z;
+    a.w += c0 * x.w + c1 * y.w + c2 * z.w;
+    q[i] = a;
+  }
+}
+__global__ void ab3_update_tail_kernel(float *__restrict__ q, const float *__restrict__ r0, const float *__restrict__ r1,
+                                       const float *__restrict__ r2, size_t begin, size_t n, float c0, float c1, float c2) {
+  const size_t i = begin + (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) q[i] += c0 * r0[i] + c1 * r1[i] + c2 * r2[i];
+}
+
+}  // namespace dgk
+
+struct dg_ctx {
+  int N = 0, Np = 0, Nfp = 0, model = 0, NF = 0, device = -1;
+  int64_t K = 0;
+  dgh::RefElem ref;
+  dgh::HostMesh mesh;
+  std::vector<double> cmax;
+  // device constants and scratch
+  float *d_DT = nullptr, *d_LT = nullptr, *d_geo = nullptr;
+  int *d_nbr = nullptr;
+  unsigned char *d_fcode = nullptr;
+  unsigned short *d_fmask = nullptr, *d_nbrnode = nullptr;
+  float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
+  int hist_head = 0;
+  // launch configuration
+  const void *k_rhs = nullptr, *k_stage = nullptr;
+  int E = 0, G = 0, NT = 0, grid = 0;
+  size_t smem = 0;
+  int last_launches = 0;
+  std::string variant;
+};
+
+namespace {
+
+template <class T>
+T *upload(const std::vector<T> &h) {
+  T *d = nullptr;
+  CUDA_TRY(cudaMalloc(&d, std::max<size_t>(h.size(), 1) * sizeof(T)));
+  CUDA_TRY(cudaMemcpy(d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return d;
+}
+
+void free_device(dg_ctx *c) {
+  if (c->device < 0) return;
+  cudaSetDevice(c->device);
+  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
+  cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
+  for (float *&h : c->d_hist) cudaFree(h);
+}
+
+void build_geo_records(const dg_ctx *c, const dg_materials *mat, std::vector<float> &geo) {
+  const int64_t K = c->K;
+  const int NG = c->model == DG_ACOUSTIC ? dgk::GEO_AC : dgk::GEO_EL;
+  geo.assign((size_t)K * NG, 0.f);
+  const dgh::HostMesh &m = c->mesh;
+  for (int64_t k = 0; k < K; ++k) {
+    float *g = &geo[(size_t)k * NG];
+    for (int i = 0; i < 9; ++i) g[i] = (float)m.G[9 * k + i];
+    const double rho = mat->rho[k], cp = mat->c_or_vp[k];
+    if (c->model == DG_ACOUSTIC) {
+      g[9] = (float)(rho * cp * cp);
+      g[10] = (float)(1.0 / rho);
+      g[11] = (float)cp;
+      const double Zm = rho * cp;
+      for (int f = 0; f < 4; ++f) {
+        const int64_t kk = m.nbr[4 * k + f] >= 0 ? m.nbr[4 * k + f] : k;
+        const double Zp = mat->rho[kk] * mat->c_or_vp[kk];
+        float *fg = g + 12 + 5 * f;
+        for (int d = 0; d < 3; ++d) fg[d] = (float)m.nrm[12 * k + 3 * f + d];
+        fg[3] = (float)(m.fscale[4 * k + f] / (Zm + Zp));   // g^sur k_c / 2, k_c = 1/{rho c}
+        fg[4] = (float)Zp;
+      }
+    } else {
+      const double cs = mat->vs[k];
+      const double mu = rho * cs * cs, lam = rho * cp * cp - 2.0 * mu;
+      g[9] = (float)(1.0 / rho);
+      g[10] = (float)lam;
+      g[11] = (float)mu;
+      g[12] = (float)cp;
+      g[13] = (float)cs;
+      for (int f = 0; f < 4; ++f) {
+        const int64_t kk = m.nbr[4 * k + f] >= 0 ? m.nbr[4 * k + f] : k;
+        const double Zpp = mat->rho[kk] * mat->c_or_vp[kk], Zsp = mat->rho[kk] * mat->vs[kk];
+        float *fg = g + 16 + 8 * f;
+        for (int d = 0; d < 3; ++d) fg[d] = (float)m.nrm[12 * k + 3 * f + d];
+        fg[3] = (float)(m.fscale[4 * k + f] / (rho * cp + Zpp));
+        fg[4] = (float)(m.fscale[4 * k + f] / (rho * cs + Zsp));
+        fg[5] = (float)Zpp;
+        fg[6] = (float)Zsp;
+      }
+    }
+  }
+}
+
+void choose_variant(dg_ctx *c, const dg_options *o) {
+  const int Np = c->Np;
+  int E = (o && o->elems_per_thread > 0) ? o->elems_per_thread : (c->model == DG_ACOUSTIC ? 4 : 2);
+  int G = (o && o->groups_per_cta > 0) ? o->groups_per_cta : std::max(1, std::min(32, (224 + Np / 2) / Np));
+  if (!(o && o->groups_per_cta > 0)) {
+    // keep the batch under ~64 KB of shared memory so several CTAs fit on an SM
+    while (G > 1 && SMEM[c->model][c->N](G * E) > 64 * 1024) --G;
+  }
+  c->k_rhs = KERNELS[c->model][c->N](E, dgk::MODE_RHS);
+  c->k_stage = KERNELS[c->model][c->N](E, dgk::MODE_STAGE);
+  if (!c->k_rhs || !c->k_stage) throw std::invalid_argument("elems_per_thread not instantiated for this model");
+  c->E = E;
+  c->G = G;
+  c->NT = ((G * Np + 31) / 32) * 32;
+  if (c->NT > 1024) throw std::invalid_argument("groups_per_cta too large: more than 1024 threads");
+  c->smem = SMEM[c->model][c->N](G * E);
+  if (c->smem > 227 * 1024) throw std::invalid_argument("batch does not fit in shared memory");
+  c->grid = (int)((c->K + (int64_t)G * E - 1) / ((int64_t)G * E));
+  char buf[128];
+  snprintf(buf, sizeof buf, "simt_fused<%s,N=%d,E=%d,G=%d,threads=%d,smem=%zu>", c->model == DG_ACOUSTIC ? "acoustic" : "elastic",
+           c->N, E, G, c->NT, c->smem);
+  c->variant = buf;
+}
+
+int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out, float *rhs, float a, float b, float dt,
+                 cudaStream_t st) {
+  dgk::StageParams p;
+  p.q_in = q_in; p.q_out = q_out; p.res = c->d_res; p.rhs = rhs;
+  p.DT = c->d_DT; p.LT = c->d_LT; p.geo = c->d_geo; p.nbr = c->d_nbr; p.fcode = c->d_fcode;
+  p.fmask = c->d_fmask; p.nbrnode = c->d_nbrnode;
+  p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
+  void *args[] = {&p};
+  cudaError_t e = cudaLaunchKernel(kernel, dim3(c->grid), dim3(c->NT), args, c->smem, st);
+  if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " launching " + c->variant);
+  return DG_OK;
+}
+
+int check_device_ctx(const dg_ctx *c) {
+  if (!c) return fail(DG_ERR_ARG, "NULL context");
+  if (c->device < 0) return fail(DG_ERR_CUDA, "host-only context: no device entry point is available (no CPU fallback)");
+  return DG_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+const char *dg_last_error(void) { return g_err.c_str(); }
+
+int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_materials *mat, const dg_options *opts) {
+  if (!out) return fail(DG_ERR_ARG, "out is NULL");
+  *out = nullptr;
+  if (!mesh || !mat || !mesh->vxyz || !mesh->etov || !mat->rho || !mat->c_or_vp) return fail(DG_ERR_ARG, "NULL input pointer");
+  if (N < 1 || N > 10) return fail(DG_ERR_ARG, "degree N must be in 1..10");
+  if (model != DG_ACOUSTIC && model != DG_ELASTIC) return fail(DG_ERR_ARG, "unknown model");
+  if (model == DG_ELASTIC && !mat->vs) return fail(DG_ERR_ARG, "elastic model needs vs");
+  if (mesh->K <= 0 || mesh->nverts <= 0) return fail(DG_ERR_MESH, "mesh: empty mesh");
+  if (mesh->K > 0x7FFFFFFF / 4) return fail(DG_ERR_MESH, "mesh: too many elements");
+  dg_ctx *c = new (std::nothrow) dg_ctx();
+  if (!c) return fail(DG_ERR_NOMEM, "out of host memory");
+  try {
+    c->N = N;
+    c->model = model;
+    c->NF = model == DG_ACOUSTIC ? 4 : 9;
+    c->K = mesh->K;
+    c->device = opts ? opts->device : 0;
+    for (int64_t k = 0; k < c->K; ++k) {
+      const double rho = mat->rho[k], cp = mat->c_or_vp[k];
+      if (!(rho > 0.0) || !(cp > 0.0) || !std::isfinite(rho) || !std::isfinite(cp)) {
+        delete c;
+        return fail(DG_ERR_MATERIAL, "material: rho and c must be positive and finite");
+      }
+      if (model == DG_ELASTIC) {
+        const double cs = mat->vs[k];
+        if (!(cs > 0.0) || !(cp > cs * std::sqrt(4.0 / 3.0))) {
+          delete c;
+          return fail(DG_ERR_MATERIAL, "material: need vs > 0 and vp > vs*sqrt(4/3)");
+        }
+      }
+    }
+    dgh::build_refelem(N, c->ref);
+    c->Np = c->ref.Np;
+    c->Nfp = c->ref.Nfp;
+    dgh::build_mesh(mesh->nverts, mesh->K, mesh->vxyz, mesh->etov, mesh->bc, c->mesh);
+    if ((double)c->K * c->NF * c->Np >= 2147483647.0 * 4) throw std::runtime_error("mesh: field array too large");
+    c->cmax.assign(mat->c_or_vp, mat->c_or_vp + c->K);
+    choose_variant(c, opts);
+    if (c->device >= 0) {
+      CUDA_TRY(cudaSetDevice(c->device));
+      const int Np = c->Np, Nfp = c->Nfp;
+      std::vector<float> DT((size_t)3 * Np * Np), LT((size_t)4 * Nfp * Np);
+      const std::vector<double> *Dm[3] = {&c->ref.Dr, &c->ref.Ds, &c->ref.Dt};
+      for (int d = 0; d < 3; ++d)
+        for (int n = 0; n < Np; ++n)
+          for (int m = 0; m < Np; ++m) DT[((size_t)d * Np + m) * Np + n] = (float)(*Dm[d])[(size_t)n * Np + m];
+      for (int n = 0; n < Np; ++n)
+        for (int j = 0; j < 4 * Nfp; ++j) LT[(size_t)j * Np + n] = (float)c->ref.LIFT[(size_t)n * 4 * Nfp + j];
+      std::vector<float> geo;
+      build_geo_records(c, mat, geo);
+      std::vector<int> nbr((size_t)4 * c->K);
+      for (size_t i = 0; i < nbr.size(); ++i) nbr[i] = c->mesh.nbr[i] >= 0 ? c->mesh.nbr[i] : -(int)c->mesh.bctag[i];
+      std::vector<unsigned short> fmask(c->ref.fmask.begin(), c->ref.fmask.end());
+      // device table indexed [f][g*6+s][i]
+      std::vector<unsigned short> nbrnode(c->ref.nbrnode.begin(), c->ref.nbrnode.end());
+      c->d_DT = upload(DT);
+      c->d_LT = upload(LT);
+      c->d_geo = upload(geo);
+      c->d_nbr = upload(nbr);
+      c->d_fcode = upload(c->mesh.fcode);
+      c->d_fmask = upload(fmask);
+      c->d_nbrnode = upload(nbrnode);
+      const size_t nq = (size_t)c->K * c->NF * Np;
+      CUDA_TRY(cudaMalloc(&c->d_res, nq * sizeof(float)));
+      CUDA_TRY(cudaMalloc(&c->d_q2, nq * sizeof(float)));
+      for (float *&h : c->d_hist) {
+        CUDA_TRY(cudaMalloc(&h, nq * sizeof(float)));
+        CUDA_TRY(cudaMemset(h, 0, nq * sizeof(float)));
+      }
+      CUDA_TRY(cudaMemset(c->d_res, 0, nq * sizeof(float)));
+      CUDA_TRY(cudaFuncSetAttribute(c->k_rhs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
+      CUDA_TRY(cudaFuncSetAttribute(c->k_stage, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
+      CUDA_TRY(cudaDeviceSynchronize());
+    }
+  } catch (const std::invalid_argument &e) {
+    free_device(c);
+    delete c;
+    return fail(DG_ERR_ARG, e.what());
+  } catch (const std::bad_alloc &) {
+    free_device(c);
+    delete c;
+    return fail(DG_ERR_NOMEM, "out of host memory");
+  } catch (const std::exception &e) {
+    const std::string msg = e.what();
+    free_device(c);
+    delete c;
+    if (msg.rfind("cuda:", 0) == 0) return fail(msg.find("out of memory") != std::string::npos ? DG_ERR_NOMEM : DG_ERR_CUDA, msg);
+    if (msg.rfind("mesh:", 0) == 0) return fail(DG_ERR_MESH, msg);
+    return fail(DG_ERR_ARG, msg);
+  }
+  *out = c;
+  return DG_OK;
+}
+
+int dg_destroy(dg_ctx *c) {
+  if (!c) return fail(DG_ERR_ARG, "NULL context");
+  free_device(c);
+  delete c;
+  return DG_OK;
+}
+
+int dg_num_fields(const dg_ctx *c) { return c ? c->NF : fail(DG_ERR_ARG, "NULL context"); }
+int dg_np(const dg_ctx *c) { return c ? c->Np : fail(DG_ERR_ARG, "NULL context"); }
+int dg_nfp(const dg_ctx *c) { return c ? c->Nfp : fail(DG_ERR_ARG, "NULL context"); }
+int64_t dg_num_elements(const dg_ctx *c) { return c ? c->K : (int64_t)fail(DG_ERR_ARG, "NULL context"); }
+int dg_last_launch_count(const dg_ctx *c) { return c ? c->last_launches : fail(DG_ERR_ARG, "NULL context"); }
+const char *dg_variant_name(const dg_ctx *c) { return c ? c->variant.c_str() : ""; }
+
+int dg_node_coords(const dg_ctx *c, double *xyz) {
+  if (!c || !xyz) return fail(DG_ERR_ARG, "NULL argument");
+  const int Np = c->Np;
+  for (int64_t k = 0; k < c->K; ++k) {
+    const double *v = &c->mesh.verts[12 * k];
+    for (int n = 0; n < Np; ++n) {
+      const double r = c->ref.r[n], s = c->ref.s[n], t = c->ref.t[n];
+      for (int d = 0; d < 3; ++d)
+        xyz[((size_t)k * Np + n) * 3 + d] = 0.5 * (-(1.0 + r + s + t) * v[d] + (1.0 + r) * v[3 + d] + (1.0 + s) * v[6 + d] + (1.0 + t) * v[9 + d]);
+    }
+  }
+  return DG_OK;
+}
+
+double dg_stable_dt(const dg_ctx *c, double cfl) {
+  if (!c || !(cfl > 0.0)) return (double)fail(DG_ERR_ARG, "bad argument");
+  double worst = 0.0;
+  for (int64_t k = 0; k < c->K; ++k) {
+    double fs = 0.0;
+    for (int f = 0; f < 4; ++f) fs = std::max(fs, c->mesh.fscale[4 * k + f]);
+    worst = std::max(worst, c->cmax[k] * fs);
+  }
+  return cfl / ((c->N + 1.0) * (c->N + 1.0) * worst);
+}
+
+int dg_reference_operators(const dg_ctx *c, double *Dr, double *Ds, double *Dt, double *LIFT, double *rst, int32_t *fmask) {
+  if (!c) return fail(DG_ERR_ARG, "NULL context");
+  const size_t nn = (size_t)c->Np * c->Np;
+  if (Dr) std::memcpy(Dr, c->ref.Dr.data(), nn * sizeof(double));
+  if (Ds) std::memcpy(Ds, c->ref.Ds.data(), nn * sizeof(double));
+  if (Dt) std::memcpy(Dt, c->ref.Dt.data(), nn * sizeof(double));
+  if (LIFT) std::memcpy(LIFT, c->ref.LIFT.data(), (size_t)c->Np * 4 * c->Nfp * sizeof(double));
+  if (rst)
+    for (int n = 0; n < c->Np; ++n) {
+      rst[3 * n + 0] = c->ref.r[n];
+      rst[3 * n + 1] = c->ref.s[n];
+      rst[3 * n + 2] = c->ref.t[n];
+    }
+  if (fmask) std::memcpy(fmask, c->ref.fmask.data(), (size_t)4 * c->Nfp * sizeof(int32_t));
+  return DG_OK;
+}
+
+int dg_geometry(const dg_ctx *c, double *G, double *J, double *nrm, double *fscale) {
+  if (!c) return fail(DG_ERR_ARG, "NULL context");
+  if (G) std::memcpy(G, c->mesh.G.data(), c->mesh.G.size() * sizeof(double));
+  if (J) std::memcpy(J, c->mesh.J.data(), c->mesh.J.size() * sizeof(double));
+  if (nrm) std::memcpy(nrm, c->mesh.nrm.data(), c->mesh.nrm.size() * sizeof(double));
+  if (fscale) std::memcpy(fscale, c->mesh.fscale.data(), c->mesh.fscale.size() * sizeof(double));
+  return DG_OK;
+}
+
+int dg_connectivity(const dg_ctx *c, int32_t *elemP, int32_t *nodeP, int8_t *bctag) {
+  if (!c) return fail(DG_ERR_ARG, "NULL context");
+  const int Nfp = c->Nfp;
+  for (int64_t k = 0; k < c->K; ++k)
+    for (int f = 0; f < 4; ++f) {
+      const int32_t nb = c->mesh.nbr[4 * k + f];
+      for (int i = 0; i < Nfp; ++i) {
+        const size_t o = ((size_t)k * 4 + f) * Nfp + i;
+        if (nb >= 0) {
+          const int code = c->mesh.fcode[4 * k + f];
+          if (elemP) elemP[o] = nb;
+          if (nodeP) nodeP[o] = c->ref.nbrnode[((size_t)f * 24 + code) * Nfp + i];
+        } else {
+          if (elemP) elemP[o] = (int32_t)k;
+          if (nodeP) nodeP[o] = c->ref.fmask[f * Nfp + i];
+        }
+      }
+      if (bctag) bctag[4 * k + f] = c->mesh.bctag[4 * k + f];
+    }
+  return DG_OK;
+}
+
+int dg_rhs(dg_ctx *c, const float *d_q, float *d_rhs, void *stream) {
+  if (int e = check_device_ctx(c)) return e;
+  if (!d_q || !d_rhs) return fail(DG_ERR_ARG, "NULL device pointer");
+  if (d_q == d_rhs) return fail(DG_ERR_ARG, "dg_rhs: d_q and d_rhs must differ");
+  c->last_launches = 1;
+  return launch_stage(c, c->k_rhs, d_q, nullptr, d_rhs, 0.f, 0.f, 0.f, (cudaStream_t)stream);
+}
+
+int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
+  if (int e = check_device_ctx(c)) return e;
+  if (!d_q || nsteps < 0) return fail(DG_ERR_ARG, "bad argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  float *cur = d_q, *oth = c->d_q2;
+  int launches = 0;
+  for (int s = 0; s < nsteps; ++s)
+    for (int i = 0; i < 5; ++i) {
+      if (int e = launch_stage(c, c->k_stage, cur, oth, nullptr, (float)RK_A[i], (float)RK_B[i], dt, st)) return e;
+      std::swap(cur, oth);
+      ++launches;
+    }
+  if (cur != d_q) {
+    cudaError_t e = cudaMemcpyAsync(d_q, cur, (size_t)c->K * c->NF * c->Np * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e));
+    ++launches;
+  }
+  c->last_launches = launches;
+  return DG_OK;
+}
+
+int dg_step(dg_ctx *c, float *d_q, float dt, void *stream) { return dg_run(c, d_q, dt, 1, stream); }
+
+int dg_ab3_reset(dg_ctx *c, void *stream) {
+  if (int e = check_device_ctx(c)) return e;
+  const size_t nq = (size_t)c->K * c->NF * c->Np;
+  for (float *h : c->d_hist)
+    if (cudaMemsetAsync(h, 0, nq * sizeof(float), (cudaStream_t)stream) != cudaSuccess) return fail(DG_ERR_CUDA, "cuda: memset failed");
+  c->hist_head = 0;
+  return DG_OK;
+}
+
+int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) {
+  if (int e = check_device_ctx(c)) return e;
+  if (!d_q) return fail(DG_ERR_ARG, "NULL device pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  // rotate history: r0 <- new, r1, r2 older (Table 1: R_0, R_-1, R_-2)
+  c->hist_head = (c->hist_head + 2) % 3;
+  float *r0 = c->d_hist[c->hist_head], *r1 = c->d_hist[(c->hist_head + 1) % 3], *r2 = c->d_hist[(c->hist_head + 2) % 3];
+  if (int e = launch_stage(c, c->k_rhs, d_q, nullptr, r0, 0.f, 0.f, 0.f, st)) return e;
+  const size_t nq = (size_t)c->K * c->NF * c->Np, n4 = nq / 4;
+  const float c0 = dt * (23.f / 12.f), c1 = dt * (-16.f / 12.f), c2 = dt * (5.f / 12.f);
+  int launches = 1;
+  if (n4) {
+    const int blocks = (int)std::min<size_t>((n4 + 255) / 256, (size_t)148 * 16);
+    dgk::ab3_update_kernel<<<blocks, 256, 0, st>>>((float4 *)d_q, (const float4 *)r0, (const float4 *)r1, (const float4 *)r2, n4, c0, c1, c2);
+    ++launches;
+  }
+  if (nq % 4) {
+    dgk::ab3_update_tail_kernel<<<1, 32, 0, st>>>(d_q, r0, r1, r2, n4 * 4, nq, c0, c1, c2);
+    ++launches;
+  }
+  if (cudaGetLastError() != cudaSuccess) return fail(DG_ERR_CUDA, "cuda: AB3 update launch failed");
+  c->last_launches = launches;
+  return DG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,35 @@
+// One translation unit per (model, degree): compiled with -DDG_MODEL=<0|1> -DDG_N=<1..10>.
+// Exposes the kernel entry points of kernels.cuh for that pair to dg_api.cu through a C getter.
+#include "kernels.cuh"
+
+#if !defined(DG_MODEL) || !defined(DG_N)
+#error "compile with -DDG_MODEL=0|1 -DDG_N=1..10"
+#endif
+
+#define DG_CAT3_(a, b, c) a##b##_##c
+#define DG_CAT3(a, b, c) DG_CAT3_(a, b, c)
+#define DG_GETTER(m, n) DG_CAT3(dgk_get_stage_kernel_, m, n)
+
+namespace {
+template <int E>
+const void *pick_mode(int mode) {
+  if (mode == dgk::MODE_RHS) return (const void *)&dgk::stage_kernel<DG_MODEL, DG_N, E, dgk::MODE_RHS>;
+  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::stage_kernel<DG_MODEL, DG_N, E, dgk::MODE_STAGE>;
+  return nullptr;
+}
+}  // namespace
+
+// returns the __global__ function for register blocking E and mode, or NULL if not instantiated
+extern "C" const void *DG_GETTER(DG_MODEL, DG_N)(int E, int mode) {
+  switch (E) {
+    case 1: return pick_mode<1>(mode);
+    case 2: return pick_mode<2>(mode);
+    case 4: return pick_mode<4>(mode);
+#if DG_MODEL == 0
+    case 8: return pick_mode<8>(mode);
+#endif
+    default: return nullptr;
+  }
+}
+
+extern "C" size_t DG_CAT3(dgk_stage_smem_bytes_, DG_MODEL, DG_N)(int EB) { return dgk::Smem<DG_MODEL, DG_N>::bytes(EB); }

@@ -1,0 +1,190 @@
+"""Thin ctypes binding over libdg.so (include/dg.h).  Argument marshalling only: every step of the
+hot path runs in the library's CUDA kernels.  PyTorch appears only in the caller, for device
+memory and streams; device buffers are passed here as raw pointers (``tensor.data_ptr()``).
+
+If libdg.so is missing the import of this module raises -- there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+ACOUSTIC, ELASTIC = 0, 1
+BC_INTERIOR, BC_RIGID, BC_FREE, BC_SLIP = 0, 1, 2, 3
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdg.so")
+if not os.path.exists(_LIB_PATH):
+    raise ImportError(f"{_LIB_PATH} not found: build it with `python -m paper_1602_07997_b200.build` "
+                      "(the product path has no CPU fallback)")
+_lib = C.CDLL(_LIB_PATH)
+
+
+class _Mesh(C.Structure):
+    _fields_ = [("nverts", C.c_int64), ("K", C.c_int64), ("vxyz", C.c_void_p), ("etov", C.c_void_p), ("bc", C.c_void_p)]
+
+
+class _Materials(C.Structure):
+    _fields_ = [("rho", C.c_void_p), ("c_or_vp", C.c_void_p), ("vs", C.c_void_p)]
+
+
+class _Options(C.Structure):
+    _fields_ = [("device", C.c_int), ("variant", C.c_int), ("elems_per_thread", C.c_int), ("groups_per_cta", C.c_int)]
+
+
+EXPORTS = ["dg_create", "dg_destroy", "dg_num_fields", "dg_np", "dg_nfp", "dg_num_elements", "dg_node_coords",
+           "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_ab3_step", "dg_ab3_reset", "dg_last_launch_count",
+           "dg_variant_name", "dg_reference_operators", "dg_geometry", "dg_connectivity", "dg_last_error"]
+
+_lib.dg_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(_Materials), C.POINTER(_Options)]
+_lib.dg_create.restype = C.c_int
+_lib.dg_destroy.argtypes = [C.c_void_p]
+for _n in ("dg_num_fields", "dg_np", "dg_nfp", "dg_last_launch_count"):
+    getattr(_lib, _n).argtypes = [C.c_void_p]
+    getattr(_lib, _n).restype = C.c_int
+_lib.dg_num_elements.argtypes = [C.c_void_p]
+_lib.dg_num_elements.restype = C.c_int64
+_lib.dg_node_coords.argtypes = [C.c_void_p, C.c_void_p]
+_lib.dg_stable_dt.argtypes = [C.c_void_p, C.c_double]
+_lib.dg_stable_dt.restype = C.c_double
+_lib.dg_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.dg_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
+_lib.dg_run.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int, C.c_void_p]
+_lib.dg_ab3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
+_lib.dg_ab3_reset.argtypes = [C.c_void_p, C.c_void_p]
+_lib.dg_variant_name.argtypes = [C.c_void_p]
+_lib.dg_variant_name.restype = C.c_char_p
+_lib.dg_reference_operators.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+_lib.dg_geometry.argtypes = [C.c_void_p] + [C.c_void_p] * 4
+_lib.dg_connectivity.argtypes = [C.c_void_p] + [C.c_void_p] * 3
+_lib.dg_last_error.restype = C.c_char_p
+
+
+class DGError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libdg error {code}: {msg}")
+        self.code = code
+
+
+def last_error() -> str:
+    return _lib.dg_last_error().decode()
+
+
+def _check(code: int) -> None:
+    if code != 0:
+        raise DGError(code, last_error())
+
+
+def _ptr(a: np.ndarray | None):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class Context:
+    """dg_create / dg_destroy pair.  Host arrays are numpy; device buffers are raw pointers (ints)."""
+
+    def __init__(self, vxyz, etov, N: int, model: int, rho, c_or_vp, vs=None, bc=None, device: int = 0,
+                 elems_per_thread: int = 0, groups_per_cta: int = 0, variant: int = 0):
+        vxyz = np.ascontiguousarray(vxyz, dtype=np.float64)
+        etov = np.ascontiguousarray(etov, dtype=np.int32)
+        bc = None if bc is None else np.ascontiguousarray(bc, dtype=np.int8)
+        rho = np.ascontiguousarray(rho, dtype=np.float64)
+        c_or_vp = np.ascontiguousarray(c_or_vp, dtype=np.float64)
+        vs = None if vs is None else np.ascontiguousarray(vs, dtype=np.float64)
+        mesh = _Mesh(vxyz.shape[0], etov.shape[0], _ptr(vxyz), _ptr(etov), _ptr(bc))
+        mat = _Materials(_ptr(rho), _ptr(c_or_vp), _ptr(vs))
+        opt = _Options(device, variant, elems_per_thread, groups_per_cta)
+        h = C.c_void_p()
+        self._h = None
+        _check(_lib.dg_create(C.byref(h), C.byref(mesh), int(N), int(model), C.byref(mat), C.byref(opt)))
+        self._h = h
+        self.N, self.model, self.device = int(N), int(model), device
+        self.K = int(_lib.dg_num_elements(h))
+        self.Np, self.Nfp, self.NF = int(_lib.dg_np(h)), int(_lib.dg_nfp(h)), int(_lib.dg_num_fields(h))
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.dg_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- host queries
+    @property
+    def shape(self):
+        return (self.K, self.NF, self.Np)
+
+    @property
+    def variant_name(self) -> str:
+        return _lib.dg_variant_name(self._h).decode()
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(_lib.dg_last_launch_count(self._h))
+
+    def node_coords(self) -> np.ndarray:
+        xyz = np.empty((self.K, self.Np, 3), dtype=np.float64)
+        _check(_lib.dg_node_coords(self._h, _ptr(xyz)))
+        return xyz
+
+    def stable_dt(self, cfl: float = 0.5) -> float:
+        dt = float(_lib.dg_stable_dt(self._h, float(cfl)))
+        if dt < 0:
+            raise DGError(int(dt), last_error())
+        return dt
+
+    def reference_operators(self):
+        Np, Nfp = self.Np, self.Nfp
+        Dr, Ds, Dt = (np.empty((Np, Np)) for _ in range(3))
+        LIFT = np.empty((Np, 4 * Nfp))
+        rst = np.empty((Np, 3))
+        fmask = np.empty((4, Nfp), dtype=np.int32)
+        _check(_lib.dg_reference_operators(self._h, _ptr(Dr), _ptr(Ds), _ptr(Dt), _ptr(LIFT), _ptr(rst), _ptr(fmask)))
+        return dict(Dr=Dr, Ds=Ds, Dt=Dt, LIFT=LIFT, rst=rst, fmask=fmask)
+
+    def geometry(self):
+        K = self.K
+        G, J, nrm, fs = np.empty((K, 3, 3)), np.empty(K), np.empty((K, 4, 3)), np.empty((K, 4))
+        _check(_lib.dg_geometry(self._h, _ptr(G), _ptr(J), _ptr(nrm), _ptr(fs)))
+        return dict(G=G, J=J, nrm=nrm, fscale=fs)
+
+    def connectivity(self):
+        K, Nfp = self.K, self.Nfp
+        eP = np.empty((K, 4 * Nfp), dtype=np.int32)
+        nP = np.empty((K, 4 * Nfp), dtype=np.int32)
+        tag = np.empty((K, 4), dtype=np.int8)
+        _check(_lib.dg_connectivity(self._h, _ptr(eP), _ptr(nP), _ptr(tag)))
+        return dict(elemP=eP, nodeP=nP, bctag=tag)
+
+    # -- device entry points (raw device pointers, cudaStream_t as int or None)
+    def rhs(self, d_q: int, d_rhs: int, stream: int | None = None):
+        _check(_lib.dg_rhs(self._h, C.c_void_p(d_q), C.c_void_p(d_rhs), C.c_void_p(stream or 0)))
+
+    def step(self, d_q: int, dt: float, stream: int | None = None):
+        _check(_lib.dg_step(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))
+
+    def run(self, d_q: int, dt: float, nsteps: int, stream: int | None = None):
+        _check(_lib.dg_run(self._h, C.c_void_p(d_q), C.c_float(dt), int(nsteps), C.c_void_p(stream or 0)))
+
+    def ab3_step(self, d_q: int, dt: float, stream: int | None = None):
+        _check(_lib.dg_ab3_step(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))
+
+    def ab3_reset(self, stream: int | None = None):
+        _check(_lib.dg_ab3_reset(self._h, C.c_void_p(stream or 0)))
+
+
+def from_workload(w, device: int = 0, **opts) -> Context:
+    """Context for a workloads.Workload (mesh, materials and boundary tags from its seeds)."""
+    vxyz, etov, bc, cell = w.mesh()
+    mats = w.material_arrays(cell)
+    if w.model == ACOUSTIC:
+        return Context(vxyz, etov, w.N, w.model, mats[0], mats[1], None, bc, device=device, **opts)
+    return Context(vxyz, etov, w.N, w.model, mats[0], mats[1], mats[2], bc, device=device, **opts)

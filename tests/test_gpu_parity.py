@@ -1,0 +1,185 @@
+"""GPU parity: libdg (CUDA, fp32, through the C ABI) against the fp64 oracle on the same seeded
+inputs.  Tolerances are BASELINE.json's: rel-L2 <= 2e-6 per RHS, <= 1e-4 after the LSRK run."""
+import numpy as np
+import pytest
+
+from paper_1602_07997_b200 import workloads as W
+
+from gpu_common import RHS_TOL, RUN_TOL, Case, rel_l2
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def dg():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_1602_07997_b200 import dg as mod          # raises if libdg.so is missing: no fallback
+    return mod
+
+
+def _sweep_case(model, N, n=3):
+    w = W.config(4, N=N, model=model, n=n)
+    w.jitter, w.top, w.ic = 0.08, W.BC_FREE, "random"
+    return w
+
+
+# ---------------------------------------------------------------- per-RHS parity, every degree, both models
+@pytest.mark.parametrize("N", range(1, 11))
+@pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
+def test_rhs_parity_all_degrees(dg, model, N):
+    """K = 162 elements (several CTAs and a ragged last batch), random N(0,1) fields, random
+    discontinuous materials, free top + rigid walls."""
+    case = Case(dg, _sweep_case(model, N))
+    q32 = case.initial_fields32()
+    got = case.gpu_rhs(torch, q32)
+    want = case.oracle_rhs(q32.astype(np.float64))
+    assert np.isfinite(got).all()
+    err = rel_l2(got, want)
+    per_field = [rel_l2(got[:, f], want[:, f]) for f in range(got.shape[1])]
+    assert err <= RHS_TOL, (case.ctx.variant_name, err, per_field)
+    assert max(per_field) <= 2 * RHS_TOL, per_field
+
+
+@pytest.mark.parametrize("model,N,E,G", [(W.ACOUSTIC, 2, 1, 5), (W.ACOUSTIC, 3, 8, 3), (W.ACOUSTIC, 4, 2, 1),
+                                         (W.ELASTIC, 2, 4, 7), (W.ELASTIC, 3, 1, 2), (W.ELASTIC, 5, 4, 1)])
+def test_rhs_parity_other_launch_shapes(dg, model, N, E, G):
+    case = Case(dg, _sweep_case(model, N), elems_per_thread=E, groups_per_cta=G)
+    q32 = case.initial_fields32()
+    err = rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64)))
+    assert err <= RHS_TOL, (case.ctx.variant_name, err)
+
+
+def test_rhs_smooth_fields_and_slip_walls(dg):
+    """Smooth data (strong cancellation in D q) and the test-only SLIP tag."""
+    w = W.config(3, n=3)
+    w.top = W.BC_SLIP
+    case = Case(dg, w)
+    q32 = case.initial_fields32()
+    assert np.abs(q32).max() > 0.1
+    err = rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64)))
+    assert err <= RHS_TOL, err
+
+
+# ---------------------------------------------------------------- config 1 exactly
+def test_config1_rhs_and_100_steps(dg):
+    case = Case(dg, W.config(1))
+    assert case.ctx.K == 384 and case.ctx.Np == 20
+    q32 = case.initial_fields32()
+    assert rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64))) <= RHS_TOL
+    dt = case.dt32()
+    got = case.gpu_run(torch, q32, dt, 100)
+    want = case.oracle_run(q32.astype(np.float64), dt, 100)
+    assert rel_l2(got, want) <= RUN_TOL
+    exact = W.standing_mode(case.mesh.x, 100 * dt)
+    assert np.abs(got - exact).max() < 1e-2                     # and it is the right physics
+
+
+# ---------------------------------------------------------------- reduced-size trajectories of configs 2, 3, 5
+@pytest.mark.parametrize("cfg,n", [(2, 6), (3, 4), (5, 2)])
+def test_trajectory_parity_reduced_configs(dg, cfg, n):
+    w = W.config(cfg, n=n)
+    case = Case(dg, w)
+    q32 = case.initial_fields32()
+    dt = case.dt32()
+    got = case.gpu_run(torch, q32, dt, w.nsteps)
+    want = case.oracle_run(q32.astype(np.float64), dt, w.nsteps)
+    assert np.isfinite(got).all()
+    assert rel_l2(got, want) <= RUN_TOL, (w.name, rel_l2(got, want))
+
+
+# ---------------------------------------------------------------- full-size configs: sampled elements
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_full_size_sampled_rhs(dg, cfg):
+    """BASELINE.json sizes in the launch configuration bench.py times; the oracle evaluates r_k on
+    sampled elements (first/last batches, boundary and interior ones) from the same global q."""
+    w = W.config(cfg)
+    K = w.K
+    rng = np.random.default_rng(cfg)
+    sample = np.unique(np.concatenate([np.arange(8), np.arange(K - 8, K), rng.integers(0, K, 48)]))
+    case = Case(dg, w, only_elems=sample)
+    q32 = case.initial_fields32()
+    if w.ic == "pulse":      # the pulse is ~0 away from the centre: sample where it lives as well
+        amp = np.abs(q32).max(axis=(1, 2))
+        hot = np.argsort(amp)[-32:]
+        sample = np.unique(np.concatenate([sample, hot]))
+        case = Case(dg, w, only_elems=sample)
+    got = case.gpu_rhs(torch, q32)[sample]
+    want = case.oracle_rhs(q32.astype(np.float64), sample)
+    assert np.isfinite(got).all()
+    assert rel_l2(got, want) <= RHS_TOL, (w.name, rel_l2(got, want))
+    # one LSRK step at full size keeps the state finite and the pulse energy bounded
+    dt = case.dt32()
+    out = case.gpu_run(torch, q32, dt, 1)
+    assert np.isfinite(out).all()
+    assert np.linalg.norm(out.astype(np.float64)) <= 1.05 * np.linalg.norm(q32.astype(np.float64))
+
+
+# ---------------------------------------------------------------- API behaviour and edge cases
+def test_edge_cases_and_api_contract(dg):
+    w = W.config(1, n=1)                                   # K = 6: less than one batch
+    case = Case(dg, w)
+    ctx = case.ctx
+    q32 = case.initial_fields32()
+    assert rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64))) <= RHS_TOL
+    d_q = torch.from_numpy(q32).cuda()
+    with pytest.raises(dg.DGError):
+        ctx.rhs(d_q.data_ptr(), d_q.data_ptr())
+    with pytest.raises(dg.DGError):
+        ctx.rhs(0, d_q.data_ptr())
+    # nsteps = 0 is a no-op
+    ctx.run(d_q.data_ptr(), 1e-3, 0)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_q.cpu().numpy(), q32) and ctx.last_launch_count == 0
+    # 2 x dg_step == dg_run(2), bit for bit; launch counts 5*n (+1 copy when odd)
+    dt = case.dt32()
+    a = case.gpu_run(torch, q32, dt, 2)
+    assert ctx.last_launch_count == 10
+    d_b = torch.from_numpy(q32).cuda()
+    ctx.step(d_b.data_ptr(), dt)
+    assert ctx.last_launch_count == 6
+    ctx.step(d_b.data_ptr(), dt)
+    torch.cuda.synchronize()
+    assert np.array_equal(a, d_b.cpu().numpy())
+    # dg_rhs does not modify q and works on a non-default stream
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        d_q2 = torch.from_numpy(q32).cuda()
+        d_r = torch.empty_like(d_q2)
+        ctx.rhs(d_q2.data_ptr(), d_r.data_ptr(), s.cuda_stream)
+    s.synchronize()
+    assert np.array_equal(d_q2.cpu().numpy(), q32)
+    assert rel_l2(d_r.cpu().numpy(), case.oracle_rhs(q32.astype(np.float64))) <= RHS_TOL
+
+
+def test_zero_field_gives_zero_rhs_and_energy_decays(dg):
+    w = _sweep_case(W.ELASTIC, 4)
+    case = Case(dg, w)
+    z = np.zeros(case.ctx.shape, dtype=np.float32)
+    assert np.all(case.gpu_rhs(torch, z) == 0)
+    from oracle import timestep
+    q32 = case.initial_fields32()
+    dt = case.dt32()
+    out = case.gpu_run(torch, q32, dt, 10).astype(np.float64)
+    e0 = timestep.energy_elastic(case.ref, case.mesh, *case.mats, q32.astype(np.float64))
+    e1 = timestep.energy_elastic(case.ref, case.mesh, *case.mats, out)
+    assert 0 < e1 < e0
+
+
+def test_ab3_matches_paper_eq4(dg):
+    """The paper's own integrator (eq. (4)): three AB3 steps from zero history."""
+    from oracle import timestep
+    case = Case(dg, W.config(1, n=2))
+    q32 = case.initial_fields32()
+    dt = case.dt32(0.2)
+    d_q = torch.from_numpy(q32).cuda()
+    case.ctx.ab3_reset()
+    for _ in range(4):
+        case.ctx.ab3_step(d_q.data_ptr(), dt)
+    torch.cuda.synchronize()
+    q = q32.astype(np.float64)
+    hist = [np.zeros_like(q), np.zeros_like(q)]
+    for _ in range(4):
+        timestep.ab3_step(q, hist, dt, case.oracle_rhs)
+    assert rel_l2(d_q.cpu().numpy(), q) <= 1e-5

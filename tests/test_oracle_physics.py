@@ -60,6 +60,7 @@ def test_negative_orientation_is_fixed(refelems):
     a = omesh.build(ref, vxyz, etov)
     b = omesh.build(ref, vxyz, flipped)
     assert np.array_equal(a.etov, b.etov) and np.all(b.J > 0)
+    assert np.array_equal(omesh.orient(vxyz, flipped)[1], np.arange(len(etov)) % 2 == 0)
 
 
 def test_nonconforming_and_untagged_meshes_raise(refelems):
