@@ -100,20 +100,28 @@ def test_full_size_sampled_rhs(dg, cfg):
     sample = np.unique(np.concatenate([np.arange(8), np.arange(K - 8, K), rng.integers(0, K, 48)]))
     case = Case(dg, w, only_elems=sample)
     q32 = case.initial_fields32()
-    if w.ic == "pulse":      # the pulse is ~0 away from the centre: sample where it lives as well
+    if w.ic == "pulse":
+        # the pulse is ~0 away from the centre, so the whole-mesh rel-L2 of BASELINE.json lives on its
+        # support: take every element that carries more than 1e-3 of the peak amplitude as well
         amp = np.abs(q32).max(axis=(1, 2))
-        hot = np.argsort(amp)[-32:]
-        sample = np.unique(np.concatenate([sample, hot]))
+        sample = np.unique(np.concatenate([sample, np.flatnonzero(amp > 1e-3 * amp.max())]))
         case = Case(dg, w, only_elems=sample)
     got = case.gpu_rhs(torch, q32)[sample]
     want = case.oracle_rhs(q32.astype(np.float64), sample)
     assert np.isfinite(got).all()
     assert rel_l2(got, want) <= RHS_TOL, (w.name, rel_l2(got, want))
-    # one LSRK step at full size keeps the state finite and the pulse energy bounded
+    # one LSRK step at full size: finite, and the discrete energy (a property that holds at any size,
+    # BASELINE.json north_star) does not grow
+    from oracle import timestep
     dt = case.dt32()
     out = case.gpu_run(torch, q32, dt, 1)
     assert np.isfinite(out).all()
-    assert np.linalg.norm(out.astype(np.float64)) <= 1.05 * np.linalg.norm(q32.astype(np.float64))
+    if w.model == W.ACOUSTIC:
+        energy = lambda q: timestep.energy_acoustic(case.ref, case.mesh, *case.mats, q)   # noqa: E731
+    else:
+        energy = lambda q: timestep.energy_elastic(case.ref, case.mesh, *case.mats, q)    # noqa: E731
+    e0, e1 = energy(q32.astype(np.float64)), energy(out.astype(np.float64))
+    assert 0 < e1 <= e0 * (1 + 1e-6), (e0, e1)
 
 
 # ---------------------------------------------------------------- API behaviour and edge cases
