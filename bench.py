@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the nodal-DG hot path (libdg, CUDA) on BASELINE.json's workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|5|4] [--N deg --model m]
+    python bench.py --impl reference ...        # the fp64 oracle on the host cores, same metric
+    python bench.py --sweep                     # config 4: every degree, both models -> JSON lines
+
+A "step" is one LSRK(5,4) time step = five fused stage kernels, each of which runs every row of
+the hot path (volume + surface + lift + update) over all K elements.  The metric is
+node-updates per second per RK stage:  K*Np*5*steps / time.
+
+Timed region: W untimed warm-up steps, then K steps bracketed by barrier + synchronize, CUDA events
+on the launching stream, max over ranks.  The state arrays (3 x K*Nf*Np floats, 1 GB for config 2)
+are larger than the 126 MB L2, so no explicit flush is needed ("l2": "inputs larger than L2").
+Multi-GPU (--gpus N under torchrun): the path has no exchange step in scope:
+N independent replicas, weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1602_07997_b200 import workloads as W  # noqa: E402
+
+METRIC = "node-updates/s per RK stage"
+UNIT = "node-updates/s"
+FP32_PEAK_TFLOPS = 72.3      # measured FFMA micro-benchmark on this pool's B200; nominal 74.5
+HBM_FALLBACK_GBS = 6650.0    # B200_PROFILING.md fallback
+
+
+def flops_per_element(model: int, N: int, with_update: bool = True) -> float:
+    """Algorithmic flops per element per RK stage (FMA = 2)."""
+    Np, Nfp = (N + 1) * (N + 2) * (N + 3) // 6, (N + 1) * (N + 2) // 2
+    if model == W.ACOUSTIC:
+        f = 12 * Np * Np + 32 * Np * Nfp + 52 * Np + 80 * Nfp
+        return f - (0 if with_update else 16 * Np)
+    f = 36 * Np * Np + 72 * Np * Nfp + 150 * Np + 400 * Nfp
+    return f - (0 if with_update else 36 * Np)
+
+
+def bytes_per_element(model: int, N: int) -> float:
+    """Compulsory HBM bytes per element per fused RK stage: read q, res; write q, res; constants."""
+    Np = (N + 1) * (N + 2) * (N + 3) // 6
+    Nf = W.NFIELDS[model]
+    geo = 128 if model == W.ACOUSTIC else 192
+    return 16 * Nf * Np + geo + 20
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured"
+    return HBM_FALLBACK_GBS, "fallback"
+
+
+def pick_workload(a) -> W.Workload:
+    if a.config == 4:
+        w = W.config(4, N=a.N or 5, model=W.ELASTIC if a.model == "elastic" else W.ACOUSTIC)
+    else:
+        w = W.config(a.config)
+    if a.cells:
+        w = W.config(a.config, N=a.N or 5, model=W.ELASTIC if a.model == "elastic" else W.ACOUSTIC, n=a.cells) \
+            if a.config == 4 else W.config(a.config, n=a.cells)
+    return w
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nme, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_run(w: W.Workload, nsteps: int, sample_elems: int, seed: int = 0):
+    """Time the fp64 oracle (as it stands) on a bounded sample of the workload: one LSRK step =
+    five evaluations of r_k on `sample_elems` elements of the full-size mesh plus the update on
+    those elements.  Returns (seconds per step, threads, description)."""
+    from oracle import mesh as omesh
+    from oracle import physics, refelem, timestep
+    ref = refelem.build(w.N)
+    vxyz, etov, bc, cell = w.mesh()
+    mats = w.material_arrays(cell)
+    K = etov.shape[0]
+    sample = np.arange(min(sample_elems, K))
+    m = omesh.build(ref, vxyz, etov, bc, only_elems=sample)
+    # neighbours of the sample may lie outside it: they are read from the global state, never updated
+    q = w.initial_fields(m.x).astype(np.float32).astype(np.float64)
+    dt = timestep.stable_dt(ref, m, mats[1])
+    if w.model == W.ACOUSTIC:
+        rhs = lambda qq: physics.rhs_acoustic(ref, m, mats[0], mats[1], qq, sample)          # noqa: E731
+    else:
+        rhs = lambda qq: physics.rhs_elastic(ref, m, *mats, qq, sample)                      # noqa: E731
+    res = np.zeros((len(sample),) + q.shape[1:])
+    times = []
+    for _ in range(nsteps):
+        t0 = time.perf_counter()
+        for A, B in zip(timestep.LSRK_A, timestep.LSRK_B):
+            res *= A
+            res += dt * rhs(q)
+            q[sample] += B * res
+        times.append(time.perf_counter() - t0)
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        threads = os.cpu_count() or 1
+    desc = f"{len(sample)} of {K} elements of {w.name}, {nsteps} LSRK step(s) = {5 * nsteps} r_k evaluations + updates, numpy fp64"
+    return times, threads, desc, len(sample)
+
+
+def run_reference(a):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = pick_workload(a)
+    per_stage_flop = flops_per_element(w.model, w.N)
+    sample_elems = a.sample or max(256, int(2.0e9 / per_stage_flop / 5))     # ~2 GFLOP per r_k evaluation
+    steps = max(1, a.steps)
+    times, threads, desc, ns = oracle_sample_run(w, a.warmup + steps, sample_elems)
+    tt = times[a.warmup:]
+    sec = sum(tt) / len(tt)
+    value = ns * w.Np * 5 / sec
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": a.gpus, "steps": steps, "warmup": a.warmup,
+        "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": w.name, "K": w.K, "N": w.N, "Np": w.Np, "stages_per_step": 5,
+                                        "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "net_gflops": ns * per_stage_flop * 5 / sec * 1e-9,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(a):
+    import torch
+    import torch.distributed as dist
+    from paper_1602_07997_b200 import dg           # raises if libdg.so is missing: no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = pick_workload(a)
+    opts = {}
+    if a.E:
+        opts["elems_per_thread"] = a.E
+    if a.G:
+        opts["groups_per_cta"] = a.G
+    ctx = dg.from_workload(w, device=local, **opts)
+    xyz = ctx.node_coords()
+    q0 = w.initial_fields(xyz).astype(np.float32)
+    del xyz
+    dt = float(np.float32(ctx.stable_dt(0.5)))
+    h_q = torch.from_numpy(q0).pin_memory()
+    d_q = h_q.cuda()
+    stream = torch.cuda.current_stream()
+    sptr = stream.cuda_stream
+
+    # ---- device-resident timing
+    for _ in range(a.warmup):
+        ctx.step(d_q.data_ptr(), dt, sptr)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    ctx.run(d_q.data_ptr(), dt, a.steps, sptr)
+    launches = ctx.last_launch_count
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if sampler else None
+    assert torch.isfinite(d_q).all().item(), "state blew up"
+
+    # ---- end to end through the C ABI with host buffers: H2D of the state, one step, D2H of the state
+    e2e_steps = max(1, min(a.steps, 5))
+    d_q.copy_(h_q, non_blocking=True)
+    ctx.step(d_q.data_ptr(), dt, sptr)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    h_out = torch.empty_like(h_q).pin_memory()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        d_q.copy_(h_q, non_blocking=True)
+        ctx.step(d_q.data_ptr(), dt, sptr)
+        h_out.copy_(d_q, non_blocking=True)
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+
+    t = torch.tensor([ms, ms_e2e], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e = float(t[0]), float(t[1])
+
+    nodes = w.K * w.Np
+    stages = 5 * a.steps
+    value = world * nodes * stages / (ms * 1e-3)
+    flops = flops_per_element(w.model, w.N) * w.K
+    byts = bytes_per_element(w.model, w.N) * w.K
+    hbm_peak, which = measured_peaks()
+    t_stage = ms * 1e-3 / stages                          # average stage-kernel duration (copy: <1/(5K) of it)
+    frac_alu = flops / t_stage / (FP32_PEAK_TFLOPS * 1e12)
+    frac_hbm = byts / t_stage / (hbm_peak * 1e9)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(w.name)
+    if frac_alu >= frac_hbm or flops / (FP32_PEAK_TFLOPS * 1e12) >= byts / (hbm_peak * 1e9):
+        roof = {"bound": "alu", "achieved": flops / t_stage * 1e-12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": frac_alu, "traffic": traffic, "peak_source": "FFMA micro-benchmark, measured (DESIGN.md)",
+                "hbm_frac": frac_hbm, "hbm_gbs": byts / t_stage * 1e-9}
+    else:
+        roof = {"bound": "hbm", "achieved": byts / t_stage * 1e-9, "peak": hbm_peak, "unit": "GB/s", "frac": frac_hbm,
+                "traffic": traffic, "peak_source": f"MEASURED_PEAKS.json ({which})", "alu_frac": frac_alu,
+                "alu_tflops": flops / t_stage * 1e-12}
+    roof["kernel"] = ctx.variant_name
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": w.name, "model": "acoustic" if w.model == W.ACOUSTIC else "elastic", "K": w.K, "N": w.N,
+                   "Np": w.Np, "stages_per_step": 5, "l2": "inputs larger than L2", "replicas": world, "dt": dt},
+        "net_gflops": world * flops * stages / (ms * 1e-3) * 1e-9,
+        "ms_per_stage": t_stage * 1e3,
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "roofline": roof,
+        "e2e": {"value": world * nodes * 5 * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": int(h_q.numel() * 4), "d2h_bytes_per_step": int(h_q.numel() * 4),
+                "steps": e2e_steps, "ms_per_step": ms_e2e / e2e_steps},
+    }
+    if rank == 0:
+        if not a.no_cpu and world == 1:
+            per_stage_flop = flops_per_element(w.model, w.N)
+            sample_elems = a.sample or max(256, int(2.0e9 / per_stage_flop / 5))
+            times, threads, desc, ns = oracle_sample_run(w, 2, sample_elems)
+            sec = times[-1]
+            line["cpu_baseline"] = {"value": ns * w.Np * 5 / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                    "sample": desc, "net_gflops_fp64": ns * per_stage_flop * 5 / sec * 1e-9}
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_sweep(a):
+    """Config 4: every degree, both models; one JSON line each (no cpu_baseline, no e2e repeat)."""
+    for model in ("acoustic", "elastic"):
+        for N in range(1, 11):
+            cmd = [sys.executable, os.path.abspath(__file__), "--config", "4", "--N", str(N), "--model", model, "--steps", str(a.steps),
+                   "--warmup", str(a.warmup), "--no-cpu"]
+            if a.cells:
+                cmd += ["--cells", str(a.cells)]
+            r = subprocess.run(cmd, capture_output=True, text=True)
+            out = [l for l in r.stdout.splitlines() if l.startswith("{")]
+            print(out[-1] if out else json.dumps({"N": N, "model": model, "error": (r.stderr or r.stdout)[-400:]}), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--N", type=int, default=None)
+    ap.add_argument("--model", default="acoustic", choices=["acoustic", "elastic"])
+    ap.add_argument("--cells", type=int, default=None, help="override cells per side (reduced sizes)")
+    ap.add_argument("--sample", type=int, default=None, help="elements in the oracle's timed sample")
+    ap.add_argument("--E", type=int, default=0)
+    ap.add_argument("--G", type=int, default=0)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sweep", action="store_true")
+    a = ap.parse_args()
+    if a.warmup < 3 and a.impl == "ours" and not a.sweep:
+        a.warmup = 3
+    if a.sweep:
+        return run_sweep(a)
+    if a.impl == "reference":
+        return run_reference(a)
+    return run_ours(a)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
