@@ -204,6 +204,8 @@ def run_ours(a):
         opts["elems_per_thread"] = a.E
     if a.G:
         opts["groups_per_cta"] = a.G
+    if a.variant:
+        opts["variant"] = a.variant
     ctx = dg.from_workload(w, device=local, **opts)
     xyz = ctx.node_coords()
     q0 = w.initial_fields(xyz).astype(np.float32)
@@ -310,6 +312,8 @@ def run_sweep(a):
                    "--warmup", str(a.warmup), "--no-cpu"]
             if a.cells:
                 cmd += ["--cells", str(a.cells)]
+            if a.variant:
+                cmd += ["--variant", str(a.variant)]
             r = subprocess.run(cmd, capture_output=True, text=True)
             out = [l for l in r.stdout.splitlines() if l.startswith("{")]
             print(out[-1] if out else json.dumps({"N": N, "model": model, "error": (r.stderr or r.stdout)[-400:]}), flush=True)
@@ -329,6 +333,7 @@ def main():
     ap.add_argument("--sample", type=int, default=None, help="elements in the oracle's timed sample")
     ap.add_argument("--E", type=int, default=0)
     ap.add_argument("--G", type=int, default=0)
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 FP32 SIMT, 2 tensor core (3xTF32)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--sweep", action="store_true")
     a = ap.parse_args()

@@ -45,8 +45,8 @@ def build(force: bool = False, jobs: int | None = None, verbose: bool = False) -
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-    hdrs = [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "host_setup.hpp"),
-            os.path.join(HERE, "..", "include", "dg.h"), os.path.abspath(__file__)]
+    hdrs = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".hpp", ".h")))
+    hdrs += [os.path.join(HERE, "..", "include", "dg.h"), os.path.abspath(__file__)]
     tasks = []
     objs = []
     for model in (0, 1):

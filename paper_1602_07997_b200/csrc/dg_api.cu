@@ -13,11 +13,13 @@
 #include "../../include/dg.h"
 #include "host_setup.hpp"
 #include "kernels.cuh"
+#include "tc_kernels.cuh"
 
 // per-(model, degree) kernel getters from stage_inst.cu
 #define DG_DECL(m, n)                                              \
   extern "C" const void *dgk_get_stage_kernel_##m##_##n(int, int); \
-  extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);
+  extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);           \
+  extern "C" const void *dgk_get_tc_kernel_##m##_##n(int);
 #define DG_DECL_ALL(m) \
   DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
 DG_DECL_ALL(0)
@@ -26,11 +28,13 @@ DG_DECL_ALL(1)
 namespace {
 typedef const void *(*kernel_getter)(int, int);
 typedef size_t (*smem_getter)(int);
+typedef const void *(*tc_getter)(int);
 #define DG_ROW(m, fn)                                                                                          \
   {nullptr, fn##m##_1, fn##m##_2, fn##m##_3, fn##m##_4, fn##m##_5, fn##m##_6, fn##m##_7, fn##m##_8, fn##m##_9, \
    fn##m##_10}
 const kernel_getter KERNELS[2][11] = {DG_ROW(0, dgk_get_stage_kernel_), DG_ROW(1, dgk_get_stage_kernel_)};
 const smem_getter SMEM[2][11] = {DG_ROW(0, dgk_stage_smem_bytes_), DG_ROW(1, dgk_stage_smem_bytes_)};
+const tc_getter TC_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc_kernel_), DG_ROW(1, dgk_get_tc_kernel_)};
 
 thread_local std::string g_err;
 int fail(int code, const std::string &msg) {
@@ -84,12 +88,15 @@ struct dg_ctx {
   int *d_nbr = nullptr;
   unsigned char *d_fcode = nullptr;
   unsigned short *d_fmask = nullptr, *d_nbrnode = nullptr;
+  float *d_Aimg = nullptr;                       // tensor-core variant: operator panel image
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
   // launch configuration
   const void *k_rhs = nullptr, *k_stage = nullptr;
   int E = 0, G = 0, NT = 0, grid = 0;
   size_t smem = 0;
+  bool tc = false;                               // tensor-core variant (tc_kernels.cuh)
+  int nbatch = 0, num_sms = 0;
   int last_launches = 0;
   std::string variant;
 };
@@ -107,7 +114,7 @@ T *upload(const std::vector<T> &h) {
 void free_device(dg_ctx *c) {
   if (c->device < 0) return;
   cudaSetDevice(c->device);
-  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
+  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Aimg); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
 }
@@ -156,7 +163,65 @@ void build_geo_records(const dg_ctx *c, const dg_materials *mat, std::vector<flo
   }
 }
 
+// round to nearest TF32 (ties away, as cvt.rna.tf32.f32): 10 explicit mantissa bits
+float tf32_rn(float x) {
+  uint32_t u;
+  std::memcpy(&u, &x, 4);
+  u = (u + 0x1000u) & 0xFFFFE000u;
+  std::memcpy(&x, &u, 4);
+  return x;
+}
+
+// Operator panel [D_r D_s D_t LIFT] of the tensor-core variant as the shared-memory image the kernel copies
+// verbatim: per stage (3 k-steps of 8) [kstep][hi|lo][k4][128 rows][4] floats, rows >= Np and k beyond the
+// panel are zero.  Node stage g: k-step j = D_j, columns 8g..8g+7; face stage: 24 columns of LIFT.
+// hi = tf32(x), lo = tf32(x - hi) from the fp64 operators (3xTF32 split, tc_kernels.cuh).
+void build_tc_image(const dgh::RefElem &ref, std::vector<float> &img) {
+  const int Np = ref.Np, NFACE = 4 * ref.Nfp;
+  const int NG = (Np + 7) / 8, NFS = (NFACE + 23) / 24;
+  img.assign((size_t)(NG + NFS) * dgk::TC_A_STAGE_FLOATS, 0.f);
+  const std::vector<double> *Dm[3] = {&ref.Dr, &ref.Ds, &ref.Dt};
+  auto put = [&](int st, int ks, int kk, int n, double v) {
+    const float hi = tf32_rn((float)v), lo = tf32_rn((float)(v - (double)hi));
+    const size_t off = (size_t)st * dgk::TC_A_STAGE_FLOATS + (size_t)(ks * 2) * dgk::TC_TILE_FLOATS + (kk >> 2) * 512 + n * 4 + (kk & 3);
+    img[off] = hi;
+    img[off + dgk::TC_TILE_FLOATS] = lo;
+  };
+  for (int st = 0; st < NG; ++st)
+    for (int ks = 0; ks < 3; ++ks)
+      for (int kk = 0; kk < 8; ++kk) {
+        const int m = 8 * st + kk;
+        if (m >= Np) continue;
+        for (int n = 0; n < Np; ++n) put(st, ks, kk, n, (*Dm[ks])[(size_t)n * Np + m]);
+      }
+  for (int fs = 0; fs < NFS; ++fs)
+    for (int ks = 0; ks < 3; ++ks)
+      for (int kk = 0; kk < 8; ++kk) {
+        const int j = fs * 24 + ks * 8 + kk;
+        if (j >= NFACE) continue;
+        for (int n = 0; n < Np; ++n) put(NG + fs, ks, kk, n, ref.LIFT[(size_t)n * NFACE + j]);
+      }
+}
+
 void choose_variant(dg_ctx *c, const dg_options *o) {
+  const int want = o ? o->variant : 0;
+  if (want < 0 || want > 2) throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core)");
+  const bool tc_ok = TC_KERNELS[c->model][c->N](dgk::MODE_STAGE) != nullptr;
+  if (want == 2 && !tc_ok) throw std::invalid_argument("tensor-core variant needs Np <= 128 (N <= 7)");
+  c->tc = want == 2;
+  if (c->tc) {
+    c->k_rhs = TC_KERNELS[c->model][c->N](dgk::MODE_RHS);
+    c->k_stage = TC_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    const int EB = dgk::TC_NCOL / c->NF;
+    c->nbatch = (int)((c->K + EB - 1) / EB);
+    c->NT = dgk::TC_THREADS;
+    c->smem = dgk::TC_SMEM_BYTES;
+    char buf[160];
+    snprintf(buf, sizeof buf, "tc_3xtf32<%s,N=%d,cols=%d,elems/batch=%d,threads=%d,smem=%zu>", c->model == DG_ACOUSTIC ? "acoustic" : "elastic",
+             c->N, dgk::TC_NCOL, EB, c->NT, c->smem);
+    c->variant = buf;
+    return;
+  }
   const int Np = c->Np;
   int E = (o && o->elems_per_thread > 0) ? o->elems_per_thread : (c->model == DG_ACOUSTIC ? 4 : 2);
   int G = (o && o->groups_per_cta > 0) ? o->groups_per_cta : std::max(1, std::min(32, (224 + Np / 2) / Np));
@@ -187,7 +252,16 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   p.DT = c->d_DT; p.LT = c->d_LT; p.geo = c->d_geo; p.nbr = c->d_nbr; p.fcode = c->d_fcode;
   p.fmask = c->d_fmask; p.nbrnode = c->d_nbrnode;
   p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
+  dgk::TcParams tp;
   void *args[] = {&p};
+  if (c->tc) {
+    // the tensor-core kernel reads node quads as float4
+    if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
+    tp.s = p;
+    tp.Aimg = c->d_Aimg;
+    tp.nbatch = c->nbatch;
+    args[0] = &tp;
+  }
   cudaError_t e = cudaLaunchKernel(kernel, dim3(c->grid), dim3(c->NT), args, c->smem, st);
   if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " launching " + c->variant);
   return DG_OK;
@@ -268,6 +342,13 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
       c->d_fcode = upload(c->mesh.fcode);
       c->d_fmask = upload(fmask);
       c->d_nbrnode = upload(nbrnode);
+      if (c->tc) {
+        std::vector<float> img;
+        build_tc_image(c->ref, img);
+        c->d_Aimg = upload(img);
+        CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
+        c->grid = std::min(c->nbatch, 2 * c->num_sms);     // persistent: 2 CTAs per SM
+      }
       const size_t nq = (size_t)c->K * c->NF * Np;
       CUDA_TRY(cudaMalloc(&c->d_res, nq * sizeof(float)));
       CUDA_TRY(cudaMalloc(&c->d_q2, nq * sizeof(float)));

@@ -13,10 +13,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-namespace dgk {
+#include "flux.cuh"
 
-constexpr int GEO_AC = 32;   // floats per element, acoustic: G[9] kappa 1/rho c | 4 x (nx ny nz fk Z+)
-constexpr int GEO_EL = 48;   // elastic: G[9] 1/rho lam mu cp cs pad pad | 4 x (nx ny nz fkp fks Zp+ Zs+ pad)
+namespace dgk {
 
 enum { MODE_RHS = 0, MODE_STAGE = 1 };
 
@@ -137,7 +136,7 @@ __global__ void stage_kernel(const StageParams p) {
     const float *qm = s_q + (e * NF) * NP + nm;
     if (MODEL == 0) {
       const float *fg = g + 12 + 5 * f;
-      const float nx = fg[0], ny = fg[1], nz = fg[2], fk = fg[3], Zp = fg[4];
+      const float nx = fg[0], ny = fg[1], nz = fg[2];
       const float pm = qm[0], vxm = qm[NP], vym = qm[2 * NP], vzm = qm[3 * NP];
       float dp, dvn;
       if (nb >= 0) {
@@ -145,77 +144,39 @@ __global__ void stage_kernel(const StageParams p) {
         const float *qp = p.q_in + ((size_t)nb * NF) * NP + nn;
         dp = __ldg(qp) - pm;
         dvn = (__ldg(qp + NP) - vxm) * nx + (__ldg(qp + 2 * NP) - vym) * ny + (__ldg(qp + 3 * NP) - vzm) * nz;
-      } else if (nb == -2) {   // free (pressure release): p+ = -p-, v+ = v-
-        dp = -2.f * pm;
-        dvn = 0.f;
-      } else {                 // rigid / slip: p+ = p-, v_n+ = -v_n-
-        dp = 0.f;
-        dvn = -2.f * (vxm * nx + vym * ny + vzm * nz);
+      } else {
+        acoustic_boundary_jump(nb, pm, vxm * nx + vym * ny + vzm * nz, dp, dvn);
       }
-      // PAPER.md:47-51 with fk = g^sur k_c / 2:  s = g^sur k_c alpha_c
-      const float sc = fk * (dp - Zp * dvn);
-      const float kap = g[9], cc = g[11];
-      float4 F;
-      F.x = kap * sc;          // -g^sur p_p
-      const float t = -cc * sc;  // -g^sur p_v
-      F.y = t * nx;
-      F.z = t * ny;
-      F.w = t * nz;
+      const float4 F = acoustic_penalty(g, fg, dp, dvn);
       s_flux[it] = (e < nvalid) ? F : make_float4(0.f, 0.f, 0.f, 0.f);
     } else {
       const float *fg = g + 16 + 8 * f;
-      const float nx = fg[0], ny = fg[1], nz = fg[2], fkp = fg[3], fks = fg[4], Zpp = fg[5], Zsp = fg[6];
+      const float nx = fg[0], ny = fg[1], nz = fg[2];
       float um[9];
 #pragma unroll
       for (int c = 0; c < 9; ++c) um[c] = qm[c * NP];
-      const float Tmx = um[3] * nx + um[6] * ny + um[7] * nz;
-      const float Tmy = um[6] * nx + um[4] * ny + um[8] * nz;
-      const float Tmz = um[7] * nx + um[8] * ny + um[5] * nz;
-      float dvx, dvy, dvz, dTx, dTy, dTz;
+      float Tmx, Tmy, Tmz;
+      traction(um, nx, ny, nz, Tmx, Tmy, Tmz);
+      float dv[3], dT[3];
       if (nb >= 0) {
         const int nn = p.nbrnode[(f * 24 + s_code[e * 4 + f]) * NFP + i];
         const float *qp = p.q_in + ((size_t)nb * NF) * NP + nn;
         float up[9];
 #pragma unroll
         for (int c = 0; c < 9; ++c) up[c] = __ldg(qp + c * NP);
-        dvx = up[0] - um[0];
-        dvy = up[1] - um[1];
-        dvz = up[2] - um[2];
-        dTx = up[3] * nx + up[6] * ny + up[7] * nz - Tmx;
-        dTy = up[6] * nx + up[4] * ny + up[8] * nz - Tmy;
-        dTz = up[7] * nx + up[8] * ny + up[5] * nz - Tmz;
-      } else if (nb == -1) {   // rigid: v+ = -v-, T+ = T-
-        dvx = -2.f * um[0]; dvy = -2.f * um[1]; dvz = -2.f * um[2];
-        dTx = dTy = dTz = 0.f;
-      } else if (nb == -2) {   // free surface: T+ = -T-, v+ = v-
-        dvx = dvy = dvz = 0.f;
-        dTx = -2.f * Tmx; dTy = -2.f * Tmy; dTz = -2.f * Tmz;
-      } else {                 // slip: v_n+ = -v_n-, T_t+ = -T_t-
-        const float vn = um[0] * nx + um[1] * ny + um[2] * nz;
-        const float Tn = Tmx * nx + Tmy * ny + Tmz * nz;
-        dvx = -2.f * vn * nx; dvy = -2.f * vn * ny; dvz = -2.f * vn * nz;
-        dTx = -2.f * (Tmx - Tn * nx); dTy = -2.f * (Tmy - Tn * ny); dTz = -2.f * (Tmz - Tn * nz);
+        float Tpx, Tpy, Tpz;
+        traction(up, nx, ny, nz, Tpx, Tpy, Tpz);
+        dv[0] = up[0] - um[0]; dv[1] = up[1] - um[1]; dv[2] = up[2] - um[2];
+        dT[0] = Tpx - Tmx; dT[1] = Tpy - Tmy; dT[2] = Tpz - Tmz;
+      } else {
+        elastic_boundary_jump(nb, um, Tmx, Tmy, Tmz, nx, ny, nz, dv, dT);
       }
-      // PAPER.md:73-84; fkp = g^sur k_p / 2, fks = g^sur k_s / 2 absorb the semi-jump halves
-      const float dTn = dTx * nx + dTy * ny + dTz * nz;
-      const float dvn = dvx * nx + dvy * ny + dvz * nz;
-      const float kpa = fkp * (dTn + Zpp * dvn);                    // g^sur k_p alpha_p
-      const float asx = fks * (dTx + Zsp * dvx), asy = fks * (dTy + Zsp * dvy), asz = fks * (dTz + Zsp * dvz);
-      const float ksa = asx * nx + asy * ny + asz * nz;             // g^sur k_s alpha_s
-      const float lam = g[10], mu = g[11], cp = g[12], cs = g[13];
-      const float cn = kpa * cp - ksa * cs;
-      const float pvx = cn * nx + cs * asx, pvy = cn * ny + cs * asy, pvz = cn * nz + cs * asz;
-      const float d0 = kpa * lam, d1 = 2.f * mu * (kpa - ksa);
-      const float Pxx = d0 + d1 * nx * nx + 2.f * mu * nx * asx;
-      const float Pyy = d0 + d1 * ny * ny + 2.f * mu * ny * asy;
-      const float Pzz = d0 + d1 * nz * nz + 2.f * mu * nz * asz;
-      const float Pxy = d1 * nx * ny + mu * (nx * asy + ny * asx);
-      const float Pxz = d1 * nx * nz + mu * (nx * asz + nz * asx);
-      const float Pyz = d1 * ny * nz + mu * (ny * asz + nz * asy);
+      float F[9];
+      elastic_penalty(g, fg, dv, dT, F);
       const bool ok = e < nvalid;
-      s_flux[it * 3 + 0] = ok ? make_float4(pvx, pvy, pvz, Pxx) : make_float4(0.f, 0.f, 0.f, 0.f);
-      s_flux[it * 3 + 1] = ok ? make_float4(Pyy, Pzz, Pxy, Pxz) : make_float4(0.f, 0.f, 0.f, 0.f);
-      s_flux[it * 3 + 2] = ok ? make_float4(Pyz, 0.f, 0.f, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+      s_flux[it * 3 + 0] = ok ? make_float4(F[0], F[1], F[2], F[3]) : make_float4(0.f, 0.f, 0.f, 0.f);
+      s_flux[it * 3 + 1] = ok ? make_float4(F[4], F[5], F[6], F[7]) : make_float4(0.f, 0.f, 0.f, 0.f);
+      s_flux[it * 3 + 2] = ok ? make_float4(F[8], 0.f, 0.f, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
   __syncthreads();

@@ -1,6 +1,7 @@
 // One translation unit per (model, degree): compiled with -DDG_MODEL=<0|1> -DDG_N=<1..10>.
 // Exposes the kernel entry points of kernels.cuh for that pair to dg_api.cu through a C getter.
 #include "kernels.cuh"
+#include "tc_kernels.cuh"
 
 #if !defined(DG_MODEL) || !defined(DG_N)
 #error "compile with -DDG_MODEL=0|1 -DDG_N=1..10"
@@ -33,3 +34,12 @@ extern "C" const void *DG_GETTER(DG_MODEL, DG_N)(int E, int mode) {
 }
 
 extern "C" size_t DG_CAT3(dgk_stage_smem_bytes_, DG_MODEL, DG_N)(int EB) { return dgk::Smem<DG_MODEL, DG_N>::bytes(EB); }
+
+// tensor-core variant (tc_kernels.cuh): one M tile, i.e. Np <= 128 (N <= 7); NULL otherwise
+extern "C" const void *DG_CAT3(dgk_get_tc_kernel_, DG_MODEL, DG_N)(int mode) {
+#if DG_N <= 7
+  if (mode == dgk::MODE_RHS) return (const void *)&dgk::tc_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
+  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::tc_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
+#endif
+  return nullptr;
+}
