@@ -14,12 +14,15 @@
 #include "host_setup.hpp"
 #include "kernels.cuh"
 #include "tc_kernels.cuh"
+#include "tc2_kernels.cuh"
 
 // per-(model, degree) kernel getters from stage_inst.cu
 #define DG_DECL(m, n)                                              \
   extern "C" const void *dgk_get_stage_kernel_##m##_##n(int, int); \
   extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);           \
-  extern "C" const void *dgk_get_tc_kernel_##m##_##n(int);
+  extern "C" const void *dgk_get_tc_kernel_##m##_##n(int);        \
+  extern "C" const void *dgk_get_tc2_kernel_##m##_##n(int);       \
+  extern "C" int dgk_tc2_info_##m##_##n(int);
 #define DG_DECL_ALL(m) \
   DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
 DG_DECL_ALL(0)
@@ -29,12 +32,15 @@ namespace {
 typedef const void *(*kernel_getter)(int, int);
 typedef size_t (*smem_getter)(int);
 typedef const void *(*tc_getter)(int);
+typedef int (*info_getter)(int);
 #define DG_ROW(m, fn)                                                                                          \
   {nullptr, fn##m##_1, fn##m##_2, fn##m##_3, fn##m##_4, fn##m##_5, fn##m##_6, fn##m##_7, fn##m##_8, fn##m##_9, \
    fn##m##_10}
 const kernel_getter KERNELS[2][11] = {DG_ROW(0, dgk_get_stage_kernel_), DG_ROW(1, dgk_get_stage_kernel_)};
 const smem_getter SMEM[2][11] = {DG_ROW(0, dgk_stage_smem_bytes_), DG_ROW(1, dgk_stage_smem_bytes_)};
 const tc_getter TC_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc_kernel_), DG_ROW(1, dgk_get_tc_kernel_)};
+const tc_getter TC2_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc2_kernel_), DG_ROW(1, dgk_get_tc2_kernel_)};
+const info_getter TC2_INFO[2][11] = {DG_ROW(0, dgk_tc2_info_), DG_ROW(1, dgk_tc2_info_)};
 
 thread_local std::string g_err;
 int fail(int code, const std::string &msg) {
@@ -88,7 +94,9 @@ struct dg_ctx {
   int *d_nbr = nullptr;
   unsigned char *d_fcode = nullptr;
   unsigned short *d_fmask = nullptr, *d_nbrnode = nullptr;
-  float *d_Aimg = nullptr;                       // tensor-core variant: operator panel image
+  float *d_Aimg = nullptr;                       // tensor-core variant 2: operator panel image
+  uint16_t *d_Bimg = nullptr;                    // tensor-core variant 3: bf16x3 operator panel image
+  bool tc2 = false;                              // warp-specialised BF16x3 variant (tc2_kernels.cuh)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
   // launch configuration
@@ -114,7 +122,7 @@ T *upload(const std::vector<T> &h) {
 void free_device(dg_ctx *c) {
   if (c->device < 0) return;
   cudaSetDevice(c->device);
-  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Aimg); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
+  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Aimg); cudaFree(c->d_Bimg); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
 }
@@ -203,9 +211,69 @@ void build_tc_image(const dgh::RefElem &ref, std::vector<float> &img) {
       }
 }
 
+// round to nearest even bf16; returns the 16-bit pattern and the value
+uint16_t bf16_rn(double x, double &val) {
+  float f = (float)x;
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  u = (u + 0x7FFFu + ((u >> 16) & 1u)) & 0xFFFF0000u;
+  std::memcpy(&f, &u, 4);
+  val = (double)f;
+  return (uint16_t)(u >> 16);
+}
+
+// Operator panel of variant 3 as the shared-memory image of every k-step (tc2_kernels.cuh):
+// [step][piece 3][kc 2][NC rows n][8 k] bf16, K-major core matrices of 8 rows x 16 bytes.  Step 3g + j holds
+// D_j[n][16g + k], step 3 NG + h holds LIFT[n][16h + k]; entries beyond Np / 4Nfp are zero.  Pieces: BF16x3
+// split of the fp64 operator entry, b1 = bf16(x), b2 = bf16(x - b1), b3 = bf16(x - b1 - b2).
+void build_tc2_image(const dgh::RefElem &ref, int NC, int nstep, std::vector<uint16_t> &img) {
+  const int Np = ref.Np, NFACE = 4 * ref.Nfp;
+  const int NG = (Np + 15) / 16;
+  const size_t stage = (size_t)3 * 2 * NC * 8;
+  img.assign((size_t)nstep * stage, 0);
+  const std::vector<double> *Dm[3] = {&ref.Dr, &ref.Ds, &ref.Dt};
+  auto put = [&](int st, int n, int k, double v) {
+    double v1, v2, v3;
+    const uint16_t b1 = bf16_rn(v, v1), b2 = bf16_rn(v - v1, v2), b3 = bf16_rn(v - v1 - v2, v3);
+    const size_t off = (size_t)st * stage + (size_t)(k >> 3) * NC * 8 + (size_t)n * 8 + (k & 7);
+    img[off] = b1;
+    img[off + (size_t)2 * NC * 8] = b2;
+    img[off + (size_t)4 * NC * 8] = b3;
+  };
+  for (int g = 0; g < NG; ++g)
+    for (int j = 0; j < 3; ++j)
+      for (int k = 0; k < 16; ++k) {
+        const int m = 16 * g + k;
+        if (m >= Np) continue;
+        for (int n = 0; n < Np; ++n) put(3 * g + j, n, k, (*Dm[j])[(size_t)n * Np + m]);
+      }
+  for (int st = 3 * NG; st < nstep; ++st)
+    for (int k = 0; k < 16; ++k) {
+      const int jf = 16 * (st - 3 * NG) + k;
+      if (jf >= NFACE) continue;
+      for (int n = 0; n < Np; ++n) put(st, n, k, ref.LIFT[(size_t)n * NFACE + jf]);
+    }
+}
+
 void choose_variant(dg_ctx *c, const dg_options *o) {
   const int want = o ? o->variant : 0;
-  if (want < 0 || want > 2) throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core)");
+  if (want < 0 || want > 3) throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core 3xTF32, 3 tensor core BF16x3)");
+  if (want == 3) {
+    if (!TC2_KERNELS[c->model][c->N](dgk::MODE_STAGE)) throw std::invalid_argument("tensor-core variant needs Np <= 128 (N <= 7)");
+    c->tc2 = true;
+    c->k_rhs = TC2_KERNELS[c->model][c->N](dgk::MODE_RHS);
+    c->k_stage = TC2_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    const info_getter info = TC2_INFO[c->model][c->N];
+    const int EB = info(1);
+    c->nbatch = (int)((c->K + EB - 1) / EB);
+    c->NT = dgk::T2_THREADS;
+    c->smem = (size_t)info(0);
+    char buf[160];
+    snprintf(buf, sizeof buf, "tc_bf16x3<%s,N=%d,NC=%d,elems/batch=%d,ksteps=%d,threads=%d,smem=%zu>",
+             c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, info(2), EB, info(3), c->NT, c->smem);
+    c->variant = buf;
+    return;
+  }
   const bool tc_ok = TC_KERNELS[c->model][c->N](dgk::MODE_STAGE) != nullptr;
   if (want == 2 && !tc_ok) throw std::invalid_argument("tensor-core variant needs Np <= 128 (N <= 7)");
   c->tc = want == 2;
@@ -253,7 +321,14 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   p.fmask = c->d_fmask; p.nbrnode = c->d_nbrnode;
   p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
   dgk::TcParams tp;
+  dgk::Tc2Params tp2;
   void *args[] = {&p};
+  if (c->tc2) {
+    tp2.s = p;
+    tp2.Bimg = c->d_Bimg;
+    tp2.nbatch = c->nbatch;
+    args[0] = &tp2;
+  }
   if (c->tc) {
     // the tensor-core kernel reads node quads as float4
     if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
@@ -342,6 +417,14 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
       c->d_fcode = upload(c->mesh.fcode);
       c->d_fmask = upload(fmask);
       c->d_nbrnode = upload(nbrnode);
+      if (c->tc2) {
+        const info_getter info = TC2_INFO[c->model][c->N];
+        std::vector<uint16_t> img;
+        build_tc2_image(c->ref, info(2), info(3), img);
+        c->d_Bimg = upload(img);
+        CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
+        c->grid = std::min(c->nbatch, c->num_sms);         // persistent: one CTA per SM
+      }
       if (c->tc) {
         std::vector<float> img;
         build_tc_image(c->ref, img);
