@@ -15,6 +15,7 @@
 #include "kernels.cuh"
 #include "tc_kernels.cuh"
 #include "tc2_kernels.cuh"
+#include "tc3_kernels.cuh"
 
 // per-(model, degree) kernel getters from stage_inst.cu
 #define DG_DECL(m, n)                                              \
@@ -22,7 +23,9 @@
   extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);           \
   extern "C" const void *dgk_get_tc_kernel_##m##_##n(int);        \
   extern "C" const void *dgk_get_tc2_kernel_##m##_##n(int);       \
-  extern "C" int dgk_tc2_info_##m##_##n(int);
+  extern "C" int dgk_tc2_info_##m##_##n(int);                     \
+  extern "C" const void *dgk_get_tc3_kernel_##m##_##n(int);       \
+  extern "C" int dgk_tc3_info_##m##_##n(int);
 #define DG_DECL_ALL(m) \
   DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
 DG_DECL_ALL(0)
@@ -41,6 +44,8 @@ const smem_getter SMEM[2][11] = {DG_ROW(0, dgk_stage_smem_bytes_), DG_ROW(1, dgk
 const tc_getter TC_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc_kernel_), DG_ROW(1, dgk_get_tc_kernel_)};
 const tc_getter TC2_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc2_kernel_), DG_ROW(1, dgk_get_tc2_kernel_)};
 const info_getter TC2_INFO[2][11] = {DG_ROW(0, dgk_tc2_info_), DG_ROW(1, dgk_tc2_info_)};
+const tc_getter TC3_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc3_kernel_), DG_ROW(1, dgk_get_tc3_kernel_)};
+const info_getter TC3_INFO[2][11] = {DG_ROW(0, dgk_tc3_info_), DG_ROW(1, dgk_tc3_info_)};
 
 thread_local std::string g_err;
 int fail(int code, const std::string &msg) {
@@ -97,6 +102,8 @@ struct dg_ctx {
   float *d_Aimg = nullptr;                       // tensor-core variant 2: operator panel image
   uint16_t *d_Bimg = nullptr;                    // tensor-core variant 3: bf16x3 operator panel image
   bool tc2 = false;                              // warp-specialised BF16x3 variant (tc2_kernels.cuh)
+  bool tc3 = false;                              // pipelined BF16x3 variant (tc3_kernels.cuh)
+  int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
   // launch configuration
@@ -122,7 +129,7 @@ T *upload(const std::vector<T> &h) {
 void free_device(dg_ctx *c) {
   if (c->device < 0) return;
   cudaSetDevice(c->device);
-  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Aimg); cudaFree(c->d_Bimg); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
+  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Aimg); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
 }
@@ -255,9 +262,59 @@ void build_tc2_image(const dgh::RefElem &ref, int NC, int nstep, std::vector<uin
     }
 }
 
+// Operator panel of variant 4 (tc3_kernels.cuh): as build_tc2_image, but the output nodes are split into NSPLIT
+// contiguous ranges of NCH rows, one image per range: [half][step][piece 3][kc 2][NCH rows n][8 k] bf16.
+void build_tc3_image(const dgh::RefElem &ref, int NCH, int nsplit, int nstep, std::vector<uint16_t> &img) {
+  const int Np = ref.Np, NFACE = 4 * ref.Nfp;
+  const int NG = (Np + 15) / 16;
+  const size_t stage = (size_t)3 * 2 * NCH * 8;
+  img.assign((size_t)nsplit * nstep * stage, 0);
+  const std::vector<double> *Dm[3] = {&ref.Dr, &ref.Ds, &ref.Dt};
+  auto put = [&](int st, int n, int k, double v) {
+    double v1, v2, v3;
+    const uint16_t b1 = bf16_rn(v, v1), b2 = bf16_rn(v - v1, v2), b3 = bf16_rn(v - v1 - v2, v3);
+    const int half = n / NCH, nn = n - half * NCH;
+    const size_t off = ((size_t)half * nstep + st) * stage + (size_t)(k >> 3) * NCH * 8 + (size_t)nn * 8 + (k & 7);
+    img[off] = b1;
+    img[off + (size_t)2 * NCH * 8] = b2;
+    img[off + (size_t)4 * NCH * 8] = b3;
+  };
+  for (int g = 0; g < NG; ++g)
+    for (int j = 0; j < 3; ++j)
+      for (int k = 0; k < 16; ++k) {
+        const int m = 16 * g + k;
+        if (m >= Np) continue;
+        for (int n = 0; n < Np; ++n) put(3 * g + j, n, k, (*Dm[j])[(size_t)n * Np + m]);
+      }
+  for (int st = 3 * NG; st < nstep; ++st)
+    for (int k = 0; k < 16; ++k) {
+      const int jf = 16 * (st - 3 * NG) + k;
+      if (jf >= NFACE) continue;
+      for (int n = 0; n < Np; ++n) put(st, n, k, ref.LIFT[(size_t)n * NFACE + jf]);
+    }
+}
+
 void choose_variant(dg_ctx *c, const dg_options *o) {
   const int want = o ? o->variant : 0;
-  if (want < 0 || want > 3) throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core 3xTF32, 3 tensor core BF16x3)");
+  if (want < 0 || want > 4)
+    throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core 3xTF32, 3 tensor core BF16x3, 4 pipelined tensor core BF16x3)");
+  if (want == 4) {
+    if (c->K >= (1 << 26)) throw std::invalid_argument("pipelined tensor-core variant packs the neighbour in 26 bits: K < 2^26");
+    c->tc3 = true;
+    c->k_rhs = TC3_KERNELS[c->model][c->N](dgk::MODE_RHS);
+    c->k_stage = TC3_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    const info_getter info = TC3_INFO[c->model][c->N];
+    const int EB = info(1);
+    c->nbatch = (int)((c->K + EB - 1) / EB);
+    c->NT = dgk::T3_THREADS;
+    c->smem = (size_t)info(0);
+    char buf[200];
+    snprintf(buf, sizeof buf, "tc_pipe_bf16x3<%s,N=%d,NCH=%d,nsplit=%d,elems/batch=%d,ksteps=%d,tile=%s x%d,accsets=%d,aring=%d,threads=%d,smem=%zu>",
+             c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, info(2), info(4), EB, info(3), info(5) ? "smem" : "L1", info(6), info(7),
+             info(8), c->NT, c->smem);
+    c->variant = buf;
+    return;
+  }
   if (want == 3) {
     if (!TC2_KERNELS[c->model][c->N](dgk::MODE_STAGE)) throw std::invalid_argument("tensor-core variant needs Np <= 128 (N <= 7)");
     c->tc2 = true;
@@ -322,7 +379,16 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
   dgk::TcParams tp;
   dgk::Tc2Params tp2;
+  dgk::Tc3Params tp3;
   void *args[] = {&p};
+  if (c->tc3) {
+    if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
+    tp3.s = p;
+    tp3.Bimg = c->d_Bimg;
+    tp3.conn = c->d_conn;
+    tp3.nbatch = c->nbatch;
+    args[0] = &tp3;
+  }
   if (c->tc2) {
     tp2.s = p;
     tp2.Bimg = c->d_Bimg;
@@ -424,6 +490,19 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         c->d_Bimg = upload(img);
         CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
         c->grid = std::min(c->nbatch, c->num_sms);         // persistent: one CTA per SM
+      }
+      if (c->tc3) {
+        const info_getter info = TC3_INFO[c->model][c->N];
+        const int nsplit = info(4);
+        std::vector<uint16_t> img;
+        build_tc3_image(c->ref, info(2), nsplit, info(3), img);
+        c->d_Bimg = upload(img);
+        std::vector<int> conn((size_t)4 * c->K);
+        for (size_t i = 0; i < conn.size(); ++i)
+          conn[i] = c->mesh.nbr[i] >= 0 ? (int)(((uint32_t)c->mesh.nbr[i] << 5) | (c->mesh.fcode[i] & 31u)) : -(int)c->mesh.bctag[i];
+        c->d_conn = upload(conn);
+        CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
+        c->grid = nsplit * std::max(1, std::min(c->nbatch, c->num_sms / nsplit));   // persistent: one CTA per SM
       }
       if (c->tc) {
         std::vector<float> img;

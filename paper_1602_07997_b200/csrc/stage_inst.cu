@@ -3,6 +3,7 @@
 #include "kernels.cuh"
 #include "tc_kernels.cuh"
 #include "tc2_kernels.cuh"
+#include "tc3_kernels.cuh"
 
 #if !defined(DG_MODEL) || !defined(DG_N)
 #error "compile with -DDG_MODEL=0|1 -DDG_N=1..10"
@@ -69,4 +70,28 @@ extern "C" int DG_CAT3(dgk_tc2_info_, DG_MODEL, DG_N)(int what) {
   (void)what;
   return -1;
 #endif
+}
+
+// pipelined warp-specialised BF16x3 tensor-core variant (tc3_kernels.cuh): every degree
+extern "C" const void *DG_CAT3(dgk_get_tc3_kernel_, DG_MODEL, DG_N)(int mode) {
+  if (mode == dgk::MODE_RHS) return (const void *)&dgk::tc3_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
+  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::tc3_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
+  return nullptr;
+}
+// launch geometry: what = 0 shared-memory bytes, 1 elements per batch, 2 NCH, 3 k-steps, 4 NSPLIT, 5 tile staged in
+// shared memory, 6 tile slots, 7 accumulator sets, 8 A ring stages
+extern "C" int DG_CAT3(dgk_tc3_info_, DG_MODEL, DG_N)(int what) {
+  using C = dgk::T3<DG_MODEL, DG_N>;
+  switch (what) {
+    case 0: return C::SMEM;
+    case 1: return C::EB;
+    case 2: return C::NCH;
+    case 3: return C::NSTEP;
+    case 4: return C::NSPLIT;
+    case 5: return C::TILE ? 1 : 0;
+    case 6: return C::NQ;
+    case 7: return C::NSETS;
+    case 8: return C::NA;
+    default: return -1;
+  }
 }

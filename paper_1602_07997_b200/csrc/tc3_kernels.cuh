@@ -1,0 +1,583 @@
+// Pipelined warp-specialised tensor-core stage kernel of libdg (sm_100a), variant 4: "tc_pipe".
+//
+// Same contraction as tc2_kernels.cuh -- per batch of 32 acoustic / 14 elastic elements (up to 128 (element,
+// field) rows = TMEM lanes)
+//
+//     R[row][n] = sum_k  A[row][k] * B[n][k]
+//
+// k = (D_j, node m): A = pre-combined (rows a1 + a3), vertex-mean shifted fields, B = D_j[n][m]  (row a2;
+// PAPER.md:171, eq. (9)-(10) P:191-204);  k = face node: A = penalty terms times g^sur (rows a4, a5), B = LIFT
+// (row a6); LSRK update (row a7) in the epilogue -- in BF16x3 split precision (six kind::f16 MMAs
+// per 16-wide k-step, two fp32 accumulators in TMEM), but with every stage of the path decoupled so that the
+// gather latency, the field-tile load and the epilogue overlap the MMAs of neighbouring batches:
+//
+//   * a loader warp streams the batch's field tile, geometric records and packed connectivity into a
+//     double-buffered shared-memory slot with bulk async copies (one batch ahead) and prefetches the batch's
+//     residual into L2 for the epilogue;
+//   * the flux warps (face gather a4 + penalty a5) work through a ring of 16-face-node chunks, several
+//     chunks -- and, with two tile slots, one batch -- ahead of the producers; exterior traces of neighbours
+//     inside the batch come from the shared-memory tile, the others from L2; all gathers of a chunk are
+//     issued before the first use;
+//   * degrees whose panel exceeds the TMEM budget (N >= 9) split the output nodes over NSPLIT = 2 CTAs
+//     (each CTA owns half of the operator rows and its own accumulators); degrees whose field tile does not
+//     fit in shared memory (N = 10) let the producers and flux warps read q through L1 instead.
+//
+// Warp roles (608 threads): 0-3 epilogue, 4-11 producers (lane = row; tcgen05.st into the TMEM A ring),
+// 12-15 flux, 16 operator stream (cp.async.bulk ring), 17 MMA issue + TMEM allocation, 18 tile loader.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "flux.cuh"
+#include "kernels.cuh"
+#include "tc_kernels.cuh"
+#include "tc2_kernels.cuh"
+
+namespace dgk {
+
+constexpr int T3_THREADS = 608;
+constexpr int T3_NB = 4;             // operator ring stages (shared memory)
+constexpr int T3_NFL = 4;            // flux chunk ring stages (shared memory)
+constexpr int T3_ASTRIDE = 24;       // TMEM columns per A stage: 3 pieces x 8 columns (16 bf16)
+constexpr int T3_FLS = 20;           // floats per row of a flux chunk (16 + pad; 80-byte rows: conflict-free float4)
+constexpr int T3_SMEM_LIMIT = 227 * 1024 - 512;
+
+template <int MODEL, int N>
+struct T3 {
+  using D = Deg<N>;
+  static constexpr int NP = D::NP, NFP = D::NFP, NFACE = D::NFACE;
+  static constexpr int NF = MODEL == 0 ? 4 : 9;
+  static constexpr int NGEO = MODEL == 0 ? GEO_AC : GEO_EL;
+  static constexpr int EB = MODEL == 0 ? 32 : 14;              // elements per batch
+  static constexpr int NR = EB * NF;                           // valid rows (<= 128)
+  static constexpr int NC = (NP + 15) / 16 * 16;               // output nodes, padded
+  static constexpr int NSPLIT = NC > 176 ? 2 : 1;              // CTAs sharing one batch (output-node halves)
+  static constexpr int NCH = NC / NSPLIT;                      // MMA N of one CTA
+  static constexpr int NG = (NP + 15) / 16;                    // node chunks of 16
+  static constexpr int NH = (NFACE + 15) / 16;                 // face-node chunks of 16
+  static constexpr int NSTEP = 3 * NG + NH;                    // k-steps of 16 per batch
+  static constexpr int NSETS = (4 * NCH + 3 * T3_ASTRIDE <= 512) ? 2 : 1;   // accumulator sets
+  static constexpr int ABASE = NSETS * 2 * NCH;                // first TMEM column of the A ring
+  static constexpr int NA_ = (512 - ABASE) / T3_ASTRIDE;
+  static constexpr int NA = NA_ > 9 ? 9 : NA_;                 // A ring stages
+  static constexpr int BSTAGE = 96 * NCH;                      // bytes: [3 pieces][2 kc][NCH][8] bf16
+  static constexpr int TILE_RAW = EB * NF * NP * 4;            // bytes of the batch's fields
+  static constexpr int META = EB * NGEO * 4 + EB * 16;         // geometric records + packed connectivity
+  static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
+  static constexpr int SCR = 4 * 32 * 33 * 4;
+  static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4;
+  static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 128;
+  static constexpr int TILE_SLOT = (TILE_RAW + 15) / 16 * 16 + 16;       // + room for a misaligned start
+  static constexpr bool TILE = FIXED + TILE_SLOT + META <= T3_SMEM_LIMIT;   // field tile staged in shared memory
+  static constexpr int NQ = !TILE ? 2 : (FIXED + 2 * (TILE_SLOT + META) <= T3_SMEM_LIMIT ? 2 : 1);
+  static constexpr int SLOT = (TILE ? TILE_SLOT : 0) + META;   // bytes of one tile slot
+  // shared-memory carve-up (bytes)
+  static constexpr int OFF_B = 0;
+  static constexpr int OFF_FLUX = OFF_B + T3_NB * BSTAGE;
+  static constexpr int OFF_SCR = OFF_FLUX + T3_NFL * FLUX_SLOT;
+  static constexpr int OFF_SLOT = OFF_SCR + SCR;
+  static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
+  static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 128;   // + slack for the 128-byte alignment
+  static constexpr int TPT = (EB * 16 + 127) / 128;            // flux tasks per thread and chunk
+  static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
+  static_assert(NA >= 3, "A ring too small");
+  static_assert(SMEM <= 227 * 1024, "shared memory");
+  static_assert(SLOT % 16 == 0 && BSTAGE % 16 == 0, "bulk copy alignment");
+};
+
+struct Tc3Params {
+  StageParams s;
+  const uint16_t *__restrict__ Bimg;   // [NSPLIT][NSTEP][3][2][NCH][8] bf16 operator panel image (host: build_tc3_image)
+  const int *__restrict__ conn;        // [K][4] packed connectivity: (neighbour << 5 | face code) or -(bc tag)
+  int nbatch;
+};
+
+namespace tc {
+__device__ __forceinline__ void prefetch_l2(const void *src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
+}
+}  // namespace tc
+
+// ---- per-row pre-combination coefficients (rows a1 + a3), record in shared memory:
+//      a_j = sum_i cf[j][i] * (u_src[i] - mean_i)
+template <int MODEL>
+__device__ __forceinline__ void row_coefficients_s(const float *g, int f, float cf[3][3], int src[3], int &nsrc) {
+  float G[9];
+#pragma unroll
+  for (int i = 0; i < 9; ++i) G[i] = g[i];
+#pragma unroll
+  for (int j = 0; j < 3; ++j)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) cf[j][i] = 0.f;
+  src[0] = src[1] = src[2] = 0;
+  if (MODEL == 0) {
+    const float kap = g[9], irho = g[10];
+    if (f == 0) {                   // eq. (5): r_p = -kappa sum_j D_j (sum_i g_ij v_i)
+      nsrc = 3;
+      src[0] = 1; src[1] = 2; src[2] = 3;
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) cf[j][i] = -kap * G[3 * i + j];
+    } else {                        // eq. (6): r_vi = -(1/rho) sum_j g_ij D_j p
+      nsrc = 1;
+#pragma unroll
+      for (int j = 0; j < 3; ++j) cf[j][0] = -irho * G[3 * (f - 1) + j];
+    }
+  } else {
+    const float irho = g[9], lam = g[10], mu = g[11];
+    nsrc = 3;
+    if (f < 3) {                    // r_vi = (1/rho) sum_j D_j (sum_m g_mj sigma_im)
+      const int row[3][3] = {{3, 6, 7}, {6, 4, 8}, {7, 8, 5}};
+#pragma unroll
+      for (int m = 0; m < 3; ++m) src[m] = row[f][m];
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int m = 0; m < 3; ++m) cf[j][m] = irho * G[3 * m + j];
+    } else {                        // PAPER.md:158 (reading Q6): lambda delta_ab div v + mu (d_b v_a + d_a v_b)
+      src[0] = 0; src[1] = 1; src[2] = 2;
+      const int a = f < 6 ? f - 3 : (f == 8 ? 1 : 0);
+      const int bb = f < 6 ? f - 3 : (f == 6 ? 1 : 2);
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        if (f < 6) {
+#pragma unroll
+          for (int i = 0; i < 3; ++i) cf[j][i] = lam * G[3 * i + j];
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          if (i == a) cf[j][i] += mu * G[3 * bb + j];
+          if (i == bb) cf[j][i] += mu * G[3 * a + j];
+        }
+      }
+    }
+  }
+}
+
+// ---- the kernel ------------------------------------------------------------------------------------
+template <int MODEL, int N, int MODE>
+__global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Params P) {
+  using C = T3<MODEL, N>;
+  constexpr int NP = C::NP, NFP = C::NFP, NFACE = C::NFACE, NF = C::NF, NGEO = C::NGEO, EB = C::EB, NCH = C::NCH;
+  constexpr int NA = C::NA, NB = T3_NB, NFL = T3_NFL, NQ = C::NQ;
+  constexpr bool TILE = C::TILE;
+  const StageParams &p = P.s;
+
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char *sm = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+  unsigned char *sB = sm + C::OFF_B;                               // [NB][3][2][NCH][8] bf16
+  float *s_flux = reinterpret_cast<float *>(sm + C::OFF_FLUX);     // [NFL][128][FLS] penalty-term chunks
+  float *s_scr = reinterpret_cast<float *>(sm + C::OFF_SCR);       // [4][32][33] epilogue transpose
+  unsigned char *s_slot = sm + C::OFF_SLOT;                        // [NQ] { field tile | geo | conn }
+  uint64_t *bars = reinterpret_cast<uint64_t *>(sm + C::OFF_BAR);
+  uint32_t *s_tmem = reinterpret_cast<uint32_t *>(bars + C::NBAR);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int hid = C::NSPLIT == 1 ? 0 : (int)(blockIdx.x % C::NSPLIT);       // which half of the output nodes
+  const int worker = (int)(blockIdx.x / C::NSPLIT), nworkers = (int)(gridDim.x / C::NSPLIT);
+  const uint32_t bar0 = tc::smem_u32(bars);
+  auto fullA = [&](int t) { return bar0 + 8u * t; };
+  auto emptyA = [&](int t) { return bar0 + 8u * (NA + t); };
+  auto fullB = [&](int t) { return bar0 + 8u * (2 * NA + t); };
+  auto emptyB = [&](int t) { return bar0 + 8u * (2 * NA + NB + t); };
+  auto flFull = [&](int t) { return bar0 + 8u * (2 * NA + 2 * NB + t); };
+  auto flEmpty = [&](int t) { return bar0 + 8u * (2 * NA + 2 * NB + NFL + t); };
+  const uint32_t barX = bar0 + 8u * (2 * NA + 2 * NB + 2 * NFL);
+  auto accFull = [&](int t) { return barX + 8u * t; };
+  auto accEmpty = [&](int t) { return barX + 8u * (2 + t); };
+  auto qFull = [&](int t) { return barX + 8u * (4 + t); };
+  auto qEmpty = [&](int t) { return barX + 8u * (6 + t); };
+  // byte offset of the batch's first field value inside its tile slot (bulk copies start 16-byte aligned)
+  auto tile_shift = [&](int k0) { return (uint32_t)(((size_t)k0 * NF * NP * 4) & 15); };
+
+  if (warp == 17) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(s_tmem)), "n"(512) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  if (tid == 0) {
+    for (int t = 0; t < NA; ++t) { tc::mbar_init(fullA(t), 8); tc::mbar_init(emptyA(t), 1); }
+    for (int t = 0; t < NB; ++t) { tc::mbar_init(fullB(t), 1); tc::mbar_init(emptyB(t), 1); }
+    for (int t = 0; t < NFL; ++t) { tc::mbar_init(flFull(t), 4); tc::mbar_init(flEmpty(t), 8); }
+    for (int t = 0; t < 2; ++t) {
+      tc::mbar_init(accFull(t), 1); tc::mbar_init(accEmpty(t), 4);
+      tc::mbar_init(qFull(t), 1); tc::mbar_init(qEmpty(t), 12);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tm = *s_tmem;
+
+  if (warp < 4) {
+    // =================================================== epilogue: LSRK update (row a7), coalesced I/O
+    const int qd = warp;
+    float *scr = s_scr + warp * (32 * 33);
+    const int n0 = hid * NCH;
+    const int ncv = min(NCH, NP - n0);                 // valid output nodes of this CTA
+    int it = 0;
+    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+      const int k0 = b * EB;
+      const int nrows = min(EB, p.K - k0) * NF;
+      const int set = C::NSETS == 2 ? (it & 1) : 0, use = C::NSETS == 2 ? (it >> 1) : it;
+      tc::mbar_wait(accFull(set), use & 1);
+      tc::tc_fence_after();
+      const uint32_t t0 = tm + ((uint32_t)(qd * 32) << 16) + set * 2 * NCH;
+      const int rmax = min(32, nrows - qd * 32);
+#pragma unroll 1
+      for (int c0 = 0; c0 < ncv; c0 += 32) {
+        uint32_t vm[32], vs[32];
+        tc::tmem_ld32(t0 + c0, vm);
+        tc::tmem_ld32(t0 + NCH + c0, vs);
+        if (c0 + 32 >= ncv) {            // accumulators drained: the MMA warp may start the next batch on this set
+          tc::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) tc::mbar_arrive(accEmpty(set));
+        }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) scr[lane * 33 + j] = __uint_as_float(vm[j]) + __uint_as_float(vs[j]);
+        __syncwarp();
+        const int nl = c0 + lane;
+        if (nl < ncv) {
+          const size_t base = ((size_t)k0 * NF + qd * 32) * NP + n0 + nl;
+#pragma unroll 8
+          for (int rr = 0; rr < rmax; ++rr) {
+            const float r = scr[rr * 33 + lane];
+            const size_t idx = base + (size_t)rr * NP;
+            if (MODE == MODE_RHS) {
+              p.rhs[idx] = r;
+            } else {
+              float rs = p.dt * r;
+              if (p.a != 0.f) rs = fmaf(p.a, p.res[idx], rs);
+              p.res[idx] = rs;
+              p.q_out[idx] = fmaf(p.b, rs, __ldg(p.q_in + idx));
+            }
+          }
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp < 12) {
+    // =================================================== producers: rows a1 + a3, BF16x3 split, tcgen05.st
+    const int pw = warp - 4, qd = pw & 3, half = pw >> 2;
+    const int r = qd * 32 + lane;                      // row = (element e, field f)
+    const int e = r / NF, f = r - e * NF;
+    const uint32_t trow = tm + ((uint32_t)(qd * 32) << 16) + C::ABASE + 4 * half;
+    constexpr bool VEC4 = (NP % 4) == 0;
+    int slot = 0;
+    uint32_t phase = 0;
+    auto emit = [&](const float *a) {                  // 8 values of this row for one k-step -> TMEM
+      uint32_t p1[4], p2[4], p3[4];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) tc::split3(a[2 * t], a[2 * t + 1], p1[t], p2[t], p3[t]);
+      tc::mbar_wait(emptyA(slot), phase ^ 1);
+      tc::tc_fence_after();
+      const uint32_t ta = trow + slot * T3_ASTRIDE;
+      tc::tmem_st4(ta, p1[0], p1[1], p1[2], p1[3]);
+      tc::tmem_st4(ta + 8, p2[0], p2[1], p2[2], p2[3]);
+      tc::tmem_st4(ta + 16, p3[0], p3[1], p3[2], p3[3]);
+      tc::tmem_st_wait();
+      tc::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(fullA(slot));
+      if (++slot == NA) { slot = 0; phase ^= 1; }
+    };
+    int it = 0, fc = 0;
+    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+      const int k0 = b * EB;
+      const int nvalid = min(EB, p.K - k0);
+      const bool valid = r < C::NR && e < nvalid;
+      const int qs = it % NQ, quse = it / NQ;
+      tc::mbar_wait(qFull(qs), quse & 1);
+      const unsigned char *sl = s_slot + qs * C::SLOT;
+      const float *s_geo = reinterpret_cast<const float *>(sl + (TILE ? C::TILE_SLOT : 0));
+      const float *qb = TILE ? reinterpret_cast<const float *>(sl + tile_shift(k0)) : p.q_in + (size_t)k0 * NF * NP;
+      auto ldq = [&](const float *x) { return TILE ? *x : __ldg(x); };
+      float cf[3][3];
+      int src[3] = {0, 0, 0}, nsrc = 0;
+      if (valid) {
+        row_coefficients_s<MODEL>(s_geo + e * NGEO, f, cf, src, nsrc);
+      } else {
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+          for (int i = 0; i < 3; ++i) cf[j][i] = 0.f;
+      }
+      const float *sp[3];
+      float mean[3];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        sp[i] = qb + (e * NF + src[i]) * NP;
+        // mean of the four vertex values: D_j 1 = 0, so the shift is exact and removes the cancellation
+        mean[i] = (valid && i < nsrc) ? 0.25f * ((ldq(sp[i]) + ldq(sp[i] + N)) + (ldq(sp[i] + C::NFP - 1) + ldq(sp[i] + NP - 1))) : 0.f;
+      }
+      auto load_u = [&](int g, float (&u)[3][8]) {
+        const int m0 = 16 * g + 8 * half;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          if (valid && i < nsrc && m0 < NP) {
+            if (VEC4) {
+#pragma unroll
+              for (int h4 = 0; h4 < 2; ++h4) {
+                if (m0 + 4 * h4 < NP) {
+                  const float4 v = TILE ? *reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4)
+                                        : __ldg(reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4));
+                  u[i][4 * h4 + 0] = v.x - mean[i]; u[i][4 * h4 + 1] = v.y - mean[i];
+                  u[i][4 * h4 + 2] = v.z - mean[i]; u[i][4 * h4 + 3] = v.w - mean[i];
+                } else {
+                  u[i][4 * h4 + 0] = u[i][4 * h4 + 1] = u[i][4 * h4 + 2] = u[i][4 * h4 + 3] = 0.f;
+                }
+              }
+            } else {
+#pragma unroll
+              for (int t = 0; t < 8; ++t) u[i][t] = (m0 + t < NP) ? ldq(sp[i] + m0 + t) - mean[i] : 0.f;
+            }
+          } else {
+#pragma unroll
+            for (int t = 0; t < 8; ++t) u[i][t] = 0.f;
+          }
+        }
+      };
+      float u[3][8];
+      if (!TILE) load_u(0, u);
+#pragma unroll 1
+      for (int g = 0; g < C::NG; ++g) {
+        float un[3][8];
+        if (TILE) {
+          load_u(g, u);
+        } else if (g + 1 < C::NG) {
+          load_u(g + 1, un);                           // global reads: one chunk ahead of its use
+        }
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+          float a[8];
+#pragma unroll
+          for (int t = 0; t < 8; ++t) a[t] = cf[j][0] * u[0][t] + cf[j][1] * u[1][t] + cf[j][2] * u[2][t];
+          emit(a);
+        }
+        if (!TILE) {
+#pragma unroll
+          for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int t = 0; t < 8; ++t) u[i][t] = un[i][t];
+        }
+      }
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(qEmpty(qs));      // this warp no longer reads the tile slot
+#pragma unroll 1
+      for (int h = 0; h < C::NH; ++h, ++fc) {
+        const int fs = fc % NFL, fuse = fc / NFL;
+        tc::mbar_wait(flFull(fs), fuse & 1);
+        const int j0 = 16 * h + 8 * half;
+        const float *fl = s_flux + fs * (128 * T3_FLS) + r * T3_FLS + 8 * half;
+        float a[8];
+        if (valid) {
+          const float4 v0 = *reinterpret_cast<const float4 *>(fl);
+          const float4 v1 = *reinterpret_cast<const float4 *>(fl + 4);
+          a[0] = v0.x; a[1] = v0.y; a[2] = v0.z; a[3] = v0.w; a[4] = v1.x; a[5] = v1.y; a[6] = v1.z; a[7] = v1.w;
+#pragma unroll
+          for (int t = 0; t < 8; ++t) a[t] = (j0 + t < NFACE) ? a[t] : 0.f;
+        } else {
+#pragma unroll
+          for (int t = 0; t < 8; ++t) a[t] = 0.f;
+        }
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(flEmpty(fs));
+        emit(a);
+      }
+    }
+  } else if (warp < 16) {
+    // =================================================== flux warps: rows a4 + a5, one 16-face-node chunk at a time
+    const int ft = tid - 384;
+    constexpr int TPT = C::TPT;
+    int it = 0, fc = 0;
+    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+      const int k0 = b * EB;
+      const int nvalid = min(EB, p.K - k0);
+      const int qs = it % NQ, quse = it / NQ;
+      tc::mbar_wait(qFull(qs), quse & 1);
+      const unsigned char *sl = s_slot + qs * C::SLOT;
+      const float *s_geo = reinterpret_cast<const float *>(sl + (TILE ? C::TILE_SLOT : 0));
+      const int *s_conn = reinterpret_cast<const int *>(s_geo + EB * NGEO);
+      const float *s_q = reinterpret_cast<const float *>(sl + tile_shift(k0));        // TILE only
+      const float *gq = p.q_in + (size_t)k0 * NF * NP;                                 // the same values in global memory
+#pragma unroll 1
+      for (int h = 0; h < C::NH; ++h, ++fc) {
+        const int fs = fc % NFL, fuse = fc / NFL;
+        // ---- gather the exterior traces of this thread's tasks (all loads in flight before the first use)
+        float ext[TPT][NF];
+        int cn[TPT];                                   // packed connectivity of the task's face; INT_MIN = no task
+#pragma unroll
+        for (int i = 0; i < TPT; ++i) {
+          const int t = ft + 128 * i;
+          const int e = t >> 4, j = 16 * h + (t & 15);
+          cn[i] = (int)0x80000000;
+#pragma unroll
+          for (int c = 0; c < NF; ++c) ext[i][c] = 0.f;
+          if (e < nvalid && j < NFACE) {
+            const int f = j / NFP;
+            const int c4 = s_conn[e * 4 + f];
+            cn[i] = c4;
+            if (c4 >= 0) {
+              const int nb = c4 >> 5;
+              const int nn = __ldg(p.nbrnode + (f * 24 + (c4 & 31)) * NFP + (j - f * NFP));
+              const unsigned rel = (unsigned)(nb - k0);
+              if (TILE && rel < (unsigned)nvalid) {    // neighbour inside the batch: its values are in the tile
+                const float *qp = s_q + (rel * NF) * NP + nn;
+#pragma unroll
+                for (int c = 0; c < NF; ++c) ext[i][c] = qp[c * NP];
+              } else {
+                const float *qp = p.q_in + ((size_t)nb * NF) * NP + nn;
+#pragma unroll
+                for (int c = 0; c < NF; ++c) ext[i][c] = __ldg(qp + c * NP);
+              }
+            }
+          }
+        }
+        tc::mbar_wait(flEmpty(fs), (fuse & 1) ^ 1);    // producers have consumed the chunk that used this slot
+        float *fl = s_flux + fs * (128 * T3_FLS);
+        // ---- penalty terms
+#pragma unroll
+        for (int i = 0; i < TPT; ++i) {
+          if (cn[i] == (int)0x80000000) continue;
+          const int t = ft + 128 * i;
+          const int e = t >> 4, jj = t & 15, j = 16 * h + jj;
+          const int f = j / NFP;
+          const float *g = s_geo + e * NGEO;
+          const int nm = __ldg(p.fmask + j);
+          float um[NF];
+          if (TILE) {
+            const float *qm = s_q + (e * NF) * NP + nm;
+#pragma unroll
+            for (int c = 0; c < NF; ++c) um[c] = qm[c * NP];
+          } else {
+            const float *qm = gq + (e * NF) * NP + nm;
+#pragma unroll
+            for (int c = 0; c < NF; ++c) um[c] = __ldg(qm + c * NP);
+          }
+          float F[NF];
+          if (MODEL == 0) {
+            const float *fg = g + 12 + 5 * f;
+            const float nx = fg[0], ny = fg[1], nz = fg[2];
+            float dp, dvn;
+            if (cn[i] >= 0) {
+              dp = ext[i][0] - um[0];
+              dvn = (ext[i][1] - um[1]) * nx + (ext[i][2] - um[2]) * ny + (ext[i][3] - um[3]) * nz;
+            } else {
+              acoustic_boundary_jump(cn[i], um[0], um[1] * nx + um[2] * ny + um[3] * nz, dp, dvn);
+            }
+            const float4 Pn = acoustic_penalty(g, fg, dp, dvn);
+            F[0] = Pn.x; F[1] = Pn.y; F[2] = Pn.z; F[3] = Pn.w;
+          } else {
+            const float *fg = g + 16 + 8 * f;
+            const float nx = fg[0], ny = fg[1], nz = fg[2];
+            float Tmx, Tmy, Tmz;
+            traction(um, nx, ny, nz, Tmx, Tmy, Tmz);
+            float dv[3], dT[3];
+            if (cn[i] >= 0) {
+              float Tpx, Tpy, Tpz;
+              traction(ext[i], nx, ny, nz, Tpx, Tpy, Tpz);
+              dv[0] = ext[i][0] - um[0]; dv[1] = ext[i][1] - um[1]; dv[2] = ext[i][2] - um[2];
+              dT[0] = Tpx - Tmx; dT[1] = Tpy - Tmy; dT[2] = Tpz - Tmz;
+            } else {
+              elastic_boundary_jump(cn[i], um, Tmx, Tmy, Tmz, nx, ny, nz, dv, dT);
+            }
+            elastic_penalty(g, fg, dv, dT, F);
+          }
+#pragma unroll
+          for (int c = 0; c < NF; ++c) fl[(e * NF + c) * T3_FLS + jj] = F[c];
+        }
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(flFull(fs));
+      }
+      __syncwarp();
+      if (lane == 0) tc::mbar_arrive(qEmpty(qs));
+    }
+  } else if (warp == 16) {
+    // =================================================== operator stream (rows a2, a6): L2 -> shared-memory ring
+    if (lane == 0) {
+      const uint16_t *img = P.Bimg + (size_t)hid * C::NSTEP * (C::BSTAGE / 2);
+      int slot = 0;
+      uint32_t phase = 0;
+      for (int b = worker; b < P.nbatch; b += nworkers) {
+        for (int st = 0; st < C::NSTEP; ++st) {
+          tc::mbar_wait(emptyB(slot), phase ^ 1);
+          tc::mbar_expect_tx(fullB(slot), C::BSTAGE);
+          tc::bulk_g2s(tc::smem_u32(sB + slot * C::BSTAGE), img + (size_t)st * (C::BSTAGE / 2), C::BSTAGE, fullB(slot));
+          if (++slot == NB) { slot = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 17) {
+    // =================================================== MMA issue: six BF16 MMAs per k-step
+    if (lane == 0) {
+      constexpr uint32_t IDESC = tc::make_idesc_bf16(128, NCH);
+      const uint64_t descB0 = tc::make_desc(tc::smem_u32(sB), NCH * 16, 128);
+      int sa = 0, sb = 0, it = 0;
+      uint32_t pa = 0, pb = 0;
+      for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+        const int set = C::NSETS == 2 ? (it & 1) : 0, use = C::NSETS == 2 ? (it >> 1) : it;
+        tc::mbar_wait(accEmpty(set), (use & 1) ^ 1);
+        tc::tc_fence_after();
+        const uint32_t d0 = tm + set * 2 * NCH, d1 = d0 + NCH;
+        for (int st = 0; st < C::NSTEP; ++st) {
+          tc::mbar_wait(fullA(sa), pa);
+          tc::mbar_wait(fullB(sb), pb);
+          tc::tc_fence_after();
+          const uint32_t a1 = tm + C::ABASE + sa * T3_ASTRIDE, a2 = a1 + 8, a3 = a1 + 16;
+          const uint64_t b1 = descB0 + (uint64_t)(sb * 6 * NCH), b2 = b1 + 2 * NCH, b3 = b2 + 2 * NCH;
+          const uint32_t acc = st > 0 ? 1u : 0u;
+          tc::umma_bf16_ts(d1, a2, b1, IDESC, acc);    // cross terms, orders 2^-8 and 2^-16
+          tc::umma_bf16_ts(d1, a1, b2, IDESC, 1u);
+          tc::umma_bf16_ts(d1, a3, b1, IDESC, 1u);
+          tc::umma_bf16_ts(d1, a2, b2, IDESC, 1u);
+          tc::umma_bf16_ts(d1, a1, b3, IDESC, 1u);
+          tc::umma_bf16_ts(d0, a1, b1, IDESC, acc);    // leading term
+          tc::umma_commit(emptyA(sa));
+          tc::umma_commit(emptyB(sb));
+          if (++sa == NA) { sa = 0; pa ^= 1; }
+          if (++sb == NB) { sb = 0; pb ^= 1; }
+        }
+        tc::umma_commit(accFull(set));
+      }
+    }
+  } else {
+    // =================================================== tile loader: fields, geometric records, connectivity
+    int it = 0;
+    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+      const int k0 = b * EB;
+      const int nvalid = min(EB, p.K - k0);
+      const int qs = it % NQ, quse = it / NQ;
+      tc::mbar_wait(qEmpty(qs), (quse & 1) ^ 1);
+      unsigned char *sl = s_slot + qs * C::SLOT;
+      // 16-byte aligned part [s_al, e_al) of the batch's byte range [s, e) of q; the (< 16 byte) tail by hand
+      const size_t s = (size_t)k0 * NF * NP * 4, e = s + (size_t)nvalid * NF * NP * 4;
+      const size_t s_al = s & ~(size_t)15, e_al = e & ~(size_t)15;
+      if (TILE) {
+        for (size_t x = e_al + 4 * lane; x < e; x += 128)
+          *reinterpret_cast<float *>(sl + (x - s_al)) = __ldg(reinterpret_cast<const float *>(reinterpret_cast<const char *>(p.q_in) + x));
+        __syncwarp();
+      }
+      if (lane == 0) {
+        const uint32_t bq = TILE ? (uint32_t)(e_al - s_al) : 0u, bg = (uint32_t)nvalid * NGEO * 4u, bc = (uint32_t)nvalid * 16u;
+        unsigned char *s_geo = sl + (TILE ? C::TILE_SLOT : 0);
+        tc::mbar_expect_tx(qFull(qs), bq + bg + bc);
+        if (TILE) tc::bulk_g2s(tc::smem_u32(sl), reinterpret_cast<const char *>(p.q_in) + s_al, bq, qFull(qs));
+        tc::bulk_g2s(tc::smem_u32(s_geo), p.geo + (size_t)k0 * NGEO, bg, qFull(qs));
+        tc::bulk_g2s(tc::smem_u32(s_geo + EB * NGEO * 4), P.conn + (size_t)k0 * 4, bc, qFull(qs));
+        if (!TILE) tc::prefetch_l2(reinterpret_cast<const char *>(p.q_in) + s_al, (uint32_t)(e_al - s_al));
+        if (MODE == MODE_STAGE && p.a != 0.f) tc::prefetch_l2(reinterpret_cast<const char *>(p.res) + s_al, (uint32_t)(e_al - s_al));
+      }
+    }
+  }
+
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  if (warp == 17) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "n"(512) : "memory");
+  }
+}
+
+}  // namespace dgk
