@@ -45,6 +45,8 @@ def build(force: bool = False, jobs: int | None = None, verbose: bool = False) -
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+    if os.environ.get("DG_PROF"):          # development: role timeline counters in the variant-4 kernel
+        flags.append("-DDG_PROF")
     hdrs = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".hpp", ".h")))
     hdrs += [os.path.join(HERE, "..", "include", "dg.h"), os.path.abspath(__file__)]
     tasks = []

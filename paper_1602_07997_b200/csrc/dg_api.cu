@@ -31,6 +31,13 @@
 DG_DECL_ALL(0)
 DG_DECL_ALL(1)
 
+#ifdef DG_PROF
+#define DG_DECLP(m, n) extern "C" int dgk_prof_read_##m##_##n(long long *);
+#define DG_DECLP_ALL(m) DG_DECLP(m, 1) DG_DECLP(m, 2) DG_DECLP(m, 3) DG_DECLP(m, 4) DG_DECLP(m, 5) DG_DECLP(m, 6) DG_DECLP(m, 7) DG_DECLP(m, 8) DG_DECLP(m, 9) DG_DECLP(m, 10)
+DG_DECLP_ALL(0)
+DG_DECLP_ALL(1)
+#endif
+
 namespace {
 typedef const void *(*kernel_getter)(int, int);
 typedef size_t (*smem_getter)(int);
@@ -694,5 +701,15 @@ int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) {
   c->last_launches = launches;
   return DG_OK;
 }
+
+#ifdef DG_PROF
+// development builds only (-DDG_PROF): per-warp wait-cycle counters of the last variant-4 launch, [296][23][5] int64
+int dg_prof_read(dg_ctx *c, long long *out) {
+  typedef int (*rd)(long long *);
+  static const rd R[2][11] = {DG_ROW(0, dgk_prof_read_), DG_ROW(1, dgk_prof_read_)};
+  cudaDeviceSynchronize();
+  return R[c->model][c->N](out);
+}
+#endif
 
 }  // extern "C"

@@ -95,3 +95,10 @@ extern "C" int DG_CAT3(dgk_tc3_info_, DG_MODEL, DG_N)(int what) {
     default: return -1;
   }
 }
+
+#ifdef DG_PROF
+// role timeline of the last tc3 launch of this (model, degree): [296][23][5] long long (tc3_kernels.cuh)
+extern "C" int DG_CAT3(dgk_prof_read_, DG_MODEL, DG_N)(long long *out) {
+  return (int)cudaMemcpyFromSymbol(out, dgk::dg_prof_buf, sizeof(dgk::dg_prof_buf));
+}
+#endif

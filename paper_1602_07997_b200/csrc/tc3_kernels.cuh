@@ -22,8 +22,8 @@
 //     (each CTA owns half of the operator rows and its own accumulators); degrees whose field tile does not
 //     fit in shared memory (N = 10) let the producers and flux warps read q through L1 instead.
 //
-// Warp roles (608 threads): 0-3 epilogue, 4-11 producers (lane = row; tcgen05.st into the TMEM A ring),
-// 12-15 flux, 16 operator stream (cp.async.bulk ring), 17 MMA issue + TMEM allocation, 18 tile loader.
+// Warp roles (736 threads): 0-3 epilogue, 4-11 producers (lane = row; tcgen05.st into the TMEM A ring),
+// 12-19 flux, 20 operator stream (cp.async.bulk ring), 21 MMA issue + TMEM allocation, 22 tile loader.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -35,7 +35,9 @@
 
 namespace dgk {
 
-constexpr int T3_THREADS = 608;
+constexpr int T3_FLUXW = 8;           // flux warps
+constexpr int T3_W_OPS = 12 + T3_FLUXW, T3_W_MMA = T3_W_OPS + 1, T3_W_LOAD = T3_W_OPS + 2;   // single-warp roles
+constexpr int T3_THREADS = (T3_W_LOAD + 1) * 32;
 constexpr int T3_NB = 4;             // operator ring stages (shared memory)
 constexpr int T3_NFL = 4;            // flux chunk ring stages (shared memory)
 constexpr int T3_ASTRIDE = 24;       // TMEM columns per A stage: 3 pieces x 8 columns (16 bf16)
@@ -64,7 +66,8 @@ struct T3 {
   static constexpr int TILE_RAW = EB * NF * NP * 4;            // bytes of the batch's fields
   static constexpr int META = EB * NGEO * 4 + EB * 16;         // geometric records + packed connectivity
   static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
-  static constexpr int SCR = 4 * 32 * 33 * 4;
+  static constexpr int CW = NC >= 128 ? 16 : 32;               // epilogue chunk width (output nodes)
+  static constexpr int SCR = 4 * 4 * 32 * (CW + 4) * 4;        // per epilogue warp: [stage 2][res | q][32][CW + 4] floats
   static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4;
   static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 128;
   static constexpr int TILE_SLOT = (TILE_RAW + 15) / 16 * 16 + 16;       // + room for a misaligned start
@@ -78,12 +81,36 @@ struct T3 {
   static constexpr int OFF_SLOT = OFF_SCR + SCR;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
   static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 128;   // + slack for the 128-byte alignment
-  static constexpr int TPT = (EB * 16 + 127) / 128;            // flux tasks per thread and chunk
+  static constexpr int TPT = (EB * 16 + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
   static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
   static_assert(NA >= 3, "A ring too small");
   static_assert(SMEM <= 227 * 1024, "shared memory");
   static_assert(SLOT % 16 == 0 && BSTAGE % 16 == 0, "bulk copy alignment");
 };
+
+// Optional role timeline (build with -DDG_PROF): every warp accumulates the cycles it spends in each kind of
+// mbarrier wait; lane 0 stores {total, wait0..wait3} per (CTA, warp) at kernel end (read back by dg_prof_read).
+#ifdef DG_PROF
+static __device__ long long dg_prof_buf[296][T3_W_LOAD + 1][5];
+#define T3_WAIT(bar, par, id)            \
+  do {                                   \
+    const long long t0_ = clock64();     \
+    tc::mbar_wait(bar, par);             \
+    prof_[id] += clock64() - t0_;        \
+  } while (0)
+#else
+#define T3_WAIT(bar, par, id) tc::mbar_wait(bar, par)
+#endif
+#ifdef DG_PROF
+#define T3_TIMED(id, stmt)              \
+  do {                                  \
+    const long long t0_ = clock64();    \
+    stmt;                               \
+    prof_[id] += clock64() - t0_;       \
+  } while (0)
+#else
+#define T3_TIMED(id, stmt) stmt
+#endif
 
 struct Tc3Params {
   StageParams s;
@@ -93,6 +120,34 @@ struct Tc3Params {
 };
 
 namespace tc {
+// one lane of the (converged) warp; ptxas keeps the code under it on the uniform datapath
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred = 0;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\t@P mov.u32 %0, 1;\n\t}\n" : "+r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ void cp_async4(uint32_t dst, const float *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(__cvta_generic_to_global(src)) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NWAIT>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NWAIT) : "memory"); }
+// 32 lanes x NCOL columns of TMEM -> NCOL registers per thread (NCOL = 16 or 32)
+template <int NCOL>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t *v) {
+  if constexpr (NCOL == 32) {
+    tmem_ld32(taddr, v);
+  } else {
+    static_assert(NCOL == 16, "16 or 32 columns");
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n\t"
+        "tcgen05.wait::ld.sync.aligned;\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+          "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+  }
+}
 __device__ __forceinline__ void prefetch_l2(const void *src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
 }
@@ -168,7 +223,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
   unsigned char *sm = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
   unsigned char *sB = sm + C::OFF_B;                               // [NB][3][2][NCH][8] bf16
   float *s_flux = reinterpret_cast<float *>(sm + C::OFF_FLUX);     // [NFL][128][FLS] penalty-term chunks
-  float *s_scr = reinterpret_cast<float *>(sm + C::OFF_SCR);       // [4][32][33] epilogue transpose
+  float *s_scr = reinterpret_cast<float *>(sm + C::OFF_SCR);       // epilogue staging (see the epilogue)
   unsigned char *s_slot = sm + C::OFF_SLOT;                        // [NQ] { field tile | geo | conn }
   uint64_t *bars = reinterpret_cast<uint64_t *>(sm + C::OFF_BAR);
   uint32_t *s_tmem = reinterpret_cast<uint32_t *>(bars + C::NBAR);
@@ -191,17 +246,17 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
   // byte offset of the batch's first field value inside its tile slot (bulk copies start 16-byte aligned)
   auto tile_shift = [&](int k0) { return (uint32_t)(((size_t)k0 * NF * NP * 4) & 15); };
 
-  if (warp == 17) {
+  if (warp == T3_W_MMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(s_tmem)), "n"(512) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   if (tid == 0) {
     for (int t = 0; t < NA; ++t) { tc::mbar_init(fullA(t), 8); tc::mbar_init(emptyA(t), 1); }
     for (int t = 0; t < NB; ++t) { tc::mbar_init(fullB(t), 1); tc::mbar_init(emptyB(t), 1); }
-    for (int t = 0; t < NFL; ++t) { tc::mbar_init(flFull(t), 4); tc::mbar_init(flEmpty(t), 8); }
+    for (int t = 0; t < NFL; ++t) { tc::mbar_init(flFull(t), T3_FLUXW); tc::mbar_init(flEmpty(t), 8); }
     for (int t = 0; t < 2; ++t) {
       tc::mbar_init(accFull(t), 1); tc::mbar_init(accEmpty(t), 4);
-      tc::mbar_init(qFull(t), 1); tc::mbar_init(qEmpty(t), 12);
+      tc::mbar_init(qFull(t), 1); tc::mbar_init(qEmpty(t), 8 + T3_FLUXW);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -209,55 +264,105 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tm = *s_tmem;
+#ifdef DG_PROF
+  long long prof_[4] = {0, 0, 0, 0};
+  const long long prof_t0 = clock64();
+#endif
 
   if (warp < 4) {
-    // =================================================== epilogue: LSRK update (row a7), coalesced I/O
+    // =================================================== epilogue: LSRK update (row a7)
+    // Chunks of 32 rows x CW output nodes.  The chunk's res / q values are brought into a per-warp staging
+    // buffer by cp.async two chunks ahead (no register or scoreboard is held while they are in flight), the
+    // update runs in the TMEM-native layout (thread = row), the results go back into the same buffer and
+    // leave through coalesced stores (lanes = consecutive nodes of one row).
+    constexpr int CW = C::CW, PITCH = CW + 4, RPI = 32 / CW;
     const int qd = warp;
-    float *scr = s_scr + warp * (32 * 33);
+    float *bufs = s_scr + warp * (4 * 32 * PITCH);     // [stage 2][res | q][32 rows][PITCH]
     const int n0 = hid * NCH;
     const int ncv = min(NCH, NP - n0);                 // valid output nodes of this CTA
-    int it = 0;
-    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
-      const int k0 = b * EB;
-      const int nrows = min(EB, p.K - k0) * NF;
-      const int set = C::NSETS == 2 ? (it & 1) : 0, use = C::NSETS == 2 ? (it >> 1) : it;
-      tc::mbar_wait(accFull(set), use & 1);
-      tc::tc_fence_after();
-      const uint32_t t0 = tm + ((uint32_t)(qd * 32) << 16) + set * 2 * NCH;
-      const int rmax = min(32, nrows - qd * 32);
-#pragma unroll 1
-      for (int c0 = 0; c0 < ncv; c0 += 32) {
-        uint32_t vm[32], vs[32];
-        tc::tmem_ld32(t0 + c0, vm);
-        tc::tmem_ld32(t0 + NCH + c0, vs);
-        if (c0 + 32 >= ncv) {            // accumulators drained: the MMA warp may start the next batch on this set
-          tc::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) tc::mbar_arrive(accEmpty(set));
+    const bool need_res = MODE == MODE_STAGE && p.a != 0.f;
+    const int sub = lane / CW, col = lane % CW;        // RPI rows per load / store instruction
+    auto issue = [&](int stg, int b, int c0) {         // async loads of chunk (b, c0) into stage stg
+      if (MODE == MODE_STAGE && b < P.nbatch && c0 + col < ncv) {
+        const int k0 = b * EB;
+        const int rmax = min(32, min(EB, p.K - k0) * NF - qd * 32);
+        const size_t base = ((size_t)k0 * NF + qd * 32) * NP + n0 + c0 + col;
+        const uint32_t dR = tc::smem_u32(bufs + (stg * 2) * 32 * PITCH + col), dQ = dR + 32 * PITCH * 4;
+#pragma unroll 4
+        for (int rr = sub; rr < rmax; rr += RPI) {
+          tc::cp_async4(dQ + rr * PITCH * 4, p.q_in + base + (size_t)rr * NP);
+          if (need_res) tc::cp_async4(dR + rr * PITCH * 4, p.res + base + (size_t)rr * NP);
         }
-#pragma unroll
-        for (int j = 0; j < 32; ++j) scr[lane * 33 + j] = __uint_as_float(vm[j]) + __uint_as_float(vs[j]);
+      }
+      tc::cp_async_commit();
+    };
+    auto advance = [&](int &b, int &c0) {
+      c0 += CW;
+      if (c0 >= ncv) { c0 = 0; b += nworkers; }
+    };
+    int ab = worker, ac0 = 0;                          // the chunk two ahead of the current one
+    issue(0, ab, ac0);
+    advance(ab, ac0);
+    issue(1, ab, ac0);
+    advance(ab, ac0);
+    int it = -1, stg = 0, set = 0;
+    for (int b = worker, c0 = 0; b < P.nbatch; advance(b, c0), stg ^= 1) {
+      const int k0 = b * EB;
+      const int rmax = min(32, min(EB, p.K - k0) * NF - qd * 32);
+      if (c0 == 0) {
+        ++it;
+        set = C::NSETS == 2 ? (it & 1) : 0;
+        T3_WAIT(accFull(set), (C::NSETS == 2 ? (it >> 1) : it) & 1, 0);
+        tc::tc_fence_after();
+      }
+      const uint32_t t0 = tm + ((uint32_t)(qd * 32) << 16) + set * 2 * NCH + c0;
+      uint32_t vm[CW], vs[CW];
+      T3_TIMED(2, tc::tmem_ld<CW>(t0, vm); tc::tmem_ld<CW>(t0 + NCH, vs));
+      if (c0 + CW >= ncv) {              // accumulators drained: the MMA warp may start the next batch on this set
+        tc::tc_fence_before();
         __syncwarp();
-        const int nl = c0 + lane;
-        if (nl < ncv) {
-          const size_t base = ((size_t)k0 * NF + qd * 32) * NP + n0 + nl;
-#pragma unroll 8
-          for (int rr = 0; rr < rmax; ++rr) {
-            const float r = scr[rr * 33 + lane];
-            const size_t idx = base + (size_t)rr * NP;
-            if (MODE == MODE_RHS) {
-              p.rhs[idx] = r;
-            } else {
-              float rs = p.dt * r;
-              if (p.a != 0.f) rs = fmaf(p.a, p.res[idx], rs);
-              p.res[idx] = rs;
-              p.q_out[idx] = fmaf(p.b, rs, __ldg(p.q_in + idx));
-            }
+        if (lane == 0) tc::mbar_arrive(accEmpty(set));
+      }
+      T3_TIMED(1, tc::cp_async_wait<1>());   // this chunk's loads have landed (the next chunk's may be in flight)
+      __syncwarp();
+      float *bR = bufs + (stg * 2) * 32 * PITCH, *bQ = bR + 32 * PITCH;
+#pragma unroll
+      for (int j4 = 0; j4 < CW / 4; ++j4) {
+        float4 *pr = reinterpret_cast<float4 *>(bR + lane * PITCH + 4 * j4), *pq = reinterpret_cast<float4 *>(bQ + lane * PITCH + 4 * j4);
+        float r[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) r[t] = __uint_as_float(vm[4 * j4 + t]) + __uint_as_float(vs[4 * j4 + t]);
+        if (MODE == MODE_RHS) {
+          *pr = make_float4(r[0], r[1], r[2], r[3]);
+        } else {
+          float4 R = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (need_res) R = *pr;
+          const float4 Q = *pq;
+          R.x = fmaf(p.a, R.x, p.dt * r[0]); R.y = fmaf(p.a, R.y, p.dt * r[1]);
+          R.z = fmaf(p.a, R.z, p.dt * r[2]); R.w = fmaf(p.a, R.w, p.dt * r[3]);
+          *pr = R;
+          *pq = make_float4(fmaf(p.b, R.x, Q.x), fmaf(p.b, R.y, Q.y), fmaf(p.b, R.z, Q.z), fmaf(p.b, R.w, Q.w));
+        }
+      }
+      __syncwarp();
+      if (c0 + col < ncv) {
+        const size_t base = ((size_t)k0 * NF + qd * 32) * NP + n0 + c0 + col;
+#pragma unroll 4
+        for (int rr = sub; rr < rmax; rr += RPI) {
+          const size_t idx = base + (size_t)rr * NP;
+          if (MODE == MODE_RHS) {
+            p.rhs[idx] = bR[rr * PITCH + col];
+          } else {
+            p.res[idx] = bR[rr * PITCH + col];
+            p.q_out[idx] = bQ[rr * PITCH + col];
           }
         }
-        __syncwarp();
       }
+      __syncwarp();
+      issue(stg, ab, ac0);
+      advance(ab, ac0);
     }
+    tc::cp_async_wait<0>();
   } else if (warp < 12) {
     // =================================================== producers: rows a1 + a3, BF16x3 split, tcgen05.st
     const int pw = warp - 4, qd = pw & 3, half = pw >> 2;
@@ -267,20 +372,30 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
     constexpr bool VEC4 = (NP % 4) == 0;
     int slot = 0;
     uint32_t phase = 0;
-    auto emit = [&](const float *a) {                  // 8 values of this row for one k-step -> TMEM
+    // One k-step of this row -> TMEM.  The completion of the tcgen05.st (wait::st, fence, arrive) of a k-step is
+    // deferred until the pieces of the next one are computed, so that its latency overlaps that arithmetic.
+    int pend = -1;                                     // A slot whose stores are in flight
+    auto finish = [&]() {
+      if (pend >= 0) {
+        tc::tmem_st_wait();
+        tc::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(fullA(pend));
+        pend = -1;
+      }
+    };
+    auto emit = [&](const float *a) {
       uint32_t p1[4], p2[4], p3[4];
 #pragma unroll
       for (int t = 0; t < 4; ++t) tc::split3(a[2 * t], a[2 * t + 1], p1[t], p2[t], p3[t]);
-      tc::mbar_wait(emptyA(slot), phase ^ 1);
+      finish();
+      T3_WAIT(emptyA(slot), phase ^ 1, 0);
       tc::tc_fence_after();
       const uint32_t ta = trow + slot * T3_ASTRIDE;
       tc::tmem_st4(ta, p1[0], p1[1], p1[2], p1[3]);
       tc::tmem_st4(ta + 8, p2[0], p2[1], p2[2], p2[3]);
       tc::tmem_st4(ta + 16, p3[0], p3[1], p3[2], p3[3]);
-      tc::tmem_st_wait();
-      tc::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) tc::mbar_arrive(fullA(slot));
+      pend = slot;
       if (++slot == NA) { slot = 0; phase ^= 1; }
     };
     int it = 0, fc = 0;
@@ -289,7 +404,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
       const int nvalid = min(EB, p.K - k0);
       const bool valid = r < C::NR && e < nvalid;
       const int qs = it % NQ, quse = it / NQ;
-      tc::mbar_wait(qFull(qs), quse & 1);
+      T3_WAIT(qFull(qs), quse & 1, 1);
       const unsigned char *sl = s_slot + qs * C::SLOT;
       const float *s_geo = reinterpret_cast<const float *>(sl + (TILE ? C::TILE_SLOT : 0));
       const float *qb = TILE ? reinterpret_cast<const float *>(sl + tile_shift(k0)) : p.q_in + (size_t)k0 * NF * NP;
@@ -368,7 +483,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
 #pragma unroll 1
       for (int h = 0; h < C::NH; ++h, ++fc) {
         const int fs = fc % NFL, fuse = fc / NFL;
-        tc::mbar_wait(flFull(fs), fuse & 1);
+        T3_WAIT(flFull(fs), fuse & 1, 2);
         const int j0 = 16 * h + 8 * half;
         const float *fl = s_flux + fs * (128 * T3_FLS) + r * T3_FLS + 8 * half;
         float a[8];
@@ -386,17 +501,18 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
         if (lane == 0) tc::mbar_arrive(flEmpty(fs));
         emit(a);
       }
+      finish();                                        // the batch's last k-step must not wait for the next batch
     }
-  } else if (warp < 16) {
+  } else if (warp < T3_W_OPS) {
     // =================================================== flux warps: rows a4 + a5, one 16-face-node chunk at a time
-    const int ft = tid - 384;
+    const int ft = tid - 384;                           // 0 .. 32 T3_FLUXW - 1
     constexpr int TPT = C::TPT;
     int it = 0, fc = 0;
     for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
       const int qs = it % NQ, quse = it / NQ;
-      tc::mbar_wait(qFull(qs), quse & 1);
+      T3_WAIT(qFull(qs), quse & 1, 0);
       const unsigned char *sl = s_slot + qs * C::SLOT;
       const float *s_geo = reinterpret_cast<const float *>(sl + (TILE ? C::TILE_SLOT : 0));
       const int *s_conn = reinterpret_cast<const int *>(s_geo + EB * NGEO);
@@ -410,7 +526,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
         int cn[TPT];                                   // packed connectivity of the task's face; INT_MIN = no task
 #pragma unroll
         for (int i = 0; i < TPT; ++i) {
-          const int t = ft + 128 * i;
+          const int t = ft + T3_FLUXW * 32 * i;
           const int e = t >> 4, j = 16 * h + (t & 15);
           cn[i] = (int)0x80000000;
 #pragma unroll
@@ -435,13 +551,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
             }
           }
         }
-        tc::mbar_wait(flEmpty(fs), (fuse & 1) ^ 1);    // producers have consumed the chunk that used this slot
+        T3_WAIT(flEmpty(fs), (fuse & 1) ^ 1, 1);    // producers have consumed the chunk that used this slot
         float *fl = s_flux + fs * (128 * T3_FLS);
         // ---- penalty terms
 #pragma unroll
         for (int i = 0; i < TPT; ++i) {
           if (cn[i] == (int)0x80000000) continue;
-          const int t = ft + 128 * i;
+          const int t = ft + T3_FLUXW * 32 * i;
           const int e = t >> 4, jj = t & 15, j = 16 * h + jj;
           const int f = j / NFP;
           const float *g = s_geo + e * NGEO;
@@ -494,37 +610,39 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
       __syncwarp();
       if (lane == 0) tc::mbar_arrive(qEmpty(qs));
     }
-  } else if (warp == 16) {
+  } else if (warp == T3_W_OPS) {
     // =================================================== operator stream (rows a2, a6): L2 -> shared-memory ring
-    if (lane == 0) {
-      const uint16_t *img = P.Bimg + (size_t)hid * C::NSTEP * (C::BSTAGE / 2);
-      int slot = 0;
-      uint32_t phase = 0;
-      for (int b = worker; b < P.nbatch; b += nworkers) {
-        for (int st = 0; st < C::NSTEP; ++st) {
-          tc::mbar_wait(emptyB(slot), phase ^ 1);
+    // (the whole warp runs the loop so that control flow stays uniform; one elected lane issues)
+    const uint16_t *img = P.Bimg + (size_t)hid * C::NSTEP * (C::BSTAGE / 2);
+    int slot = 0;
+    uint32_t phase = 0;
+    for (int b = worker; b < P.nbatch; b += nworkers) {
+      for (int st = 0; st < C::NSTEP; ++st) {
+        T3_WAIT(emptyB(slot), phase ^ 1, 0);
+        if (tc::elect_one()) {
           tc::mbar_expect_tx(fullB(slot), C::BSTAGE);
           tc::bulk_g2s(tc::smem_u32(sB + slot * C::BSTAGE), img + (size_t)st * (C::BSTAGE / 2), C::BSTAGE, fullB(slot));
-          if (++slot == NB) { slot = 0; phase ^= 1; }
         }
+        __syncwarp();
+        if (++slot == NB) { slot = 0; phase ^= 1; }
       }
     }
-  } else if (warp == 17) {
+  } else if (warp == T3_W_MMA) {
     // =================================================== MMA issue: six BF16 MMAs per k-step
-    if (lane == 0) {
-      constexpr uint32_t IDESC = tc::make_idesc_bf16(128, NCH);
-      const uint64_t descB0 = tc::make_desc(tc::smem_u32(sB), NCH * 16, 128);
-      int sa = 0, sb = 0, it = 0;
-      uint32_t pa = 0, pb = 0;
-      for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
-        const int set = C::NSETS == 2 ? (it & 1) : 0, use = C::NSETS == 2 ? (it >> 1) : it;
-        tc::mbar_wait(accEmpty(set), (use & 1) ^ 1);
+    constexpr uint32_t IDESC = tc::make_idesc_bf16(128, NCH);
+    const uint64_t descB0 = tc::make_desc(tc::smem_u32(sB), NCH * 16, 128);
+    int sa = 0, sb = 0, it = 0;
+    uint32_t pa = 0, pb = 0;
+    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+      const int set = C::NSETS == 2 ? (it & 1) : 0, use = C::NSETS == 2 ? (it >> 1) : it;
+      T3_WAIT(accEmpty(set), (use & 1) ^ 1, 0);
+      tc::tc_fence_after();
+      const uint32_t d0 = tm + set * 2 * NCH, d1 = d0 + NCH;
+      for (int st = 0; st < C::NSTEP; ++st) {
+        T3_WAIT(fullA(sa), pa, 1);
+        T3_WAIT(fullB(sb), pb, 2);
         tc::tc_fence_after();
-        const uint32_t d0 = tm + set * 2 * NCH, d1 = d0 + NCH;
-        for (int st = 0; st < C::NSTEP; ++st) {
-          tc::mbar_wait(fullA(sa), pa);
-          tc::mbar_wait(fullB(sb), pb);
-          tc::tc_fence_after();
+        if (tc::elect_one()) {
           const uint32_t a1 = tm + C::ABASE + sa * T3_ASTRIDE, a2 = a1 + 8, a3 = a1 + 16;
           const uint64_t b1 = descB0 + (uint64_t)(sb * 6 * NCH), b2 = b1 + 2 * NCH, b3 = b2 + 2 * NCH;
           const uint32_t acc = st > 0 ? 1u : 0u;
@@ -536,10 +654,11 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
           tc::umma_bf16_ts(d0, a1, b1, IDESC, acc);    // leading term
           tc::umma_commit(emptyA(sa));
           tc::umma_commit(emptyB(sb));
-          if (++sa == NA) { sa = 0; pa ^= 1; }
-          if (++sb == NB) { sb = 0; pb ^= 1; }
+          if (st == C::NSTEP - 1) tc::umma_commit(accFull(set));
         }
-        tc::umma_commit(accFull(set));
+        __syncwarp();
+        if (++sa == NA) { sa = 0; pa ^= 1; }
+        if (++sb == NB) { sb = 0; pb ^= 1; }
       }
     }
   } else {
@@ -549,7 +668,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
       const int qs = it % NQ, quse = it / NQ;
-      tc::mbar_wait(qEmpty(qs), (quse & 1) ^ 1);
+      T3_WAIT(qEmpty(qs), (quse & 1) ^ 1, 0);
       unsigned char *sl = s_slot + qs * C::SLOT;
       // 16-byte aligned part [s_al, e_al) of the batch's byte range [s, e) of q; the (< 16 byte) tail by hand
       const size_t s = (size_t)k0 * NF * NP * 4, e = s + (size_t)nvalid * NF * NP * 4;
@@ -572,10 +691,17 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
     }
   }
 
+#ifdef DG_PROF
+  if (lane == 0 && blockIdx.x < 296) {
+    long long *o = dg_prof_buf[blockIdx.x][warp];
+    o[0] = clock64() - prof_t0;
+    for (int i = 0; i < 4; ++i) o[1 + i] = prof_[i];
+  }
+#endif
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
-  if (warp == 17) {
+  if (warp == T3_W_MMA) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm), "n"(512) : "memory");
   }
 }
