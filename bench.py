@@ -58,11 +58,13 @@ def bytes_per_element(model: int, N: int) -> float:
 
 
 def measured_peaks():
+    """(HBM GB/s, dense bf16 TFLOP/s sustained, source).  The stage kernels run back to back inside a long
+    step, so the sustained tensor figure is the one that applies (B200_PROFILING.md)."""
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
-        return float(d["hbm_gbs"]), "measured"
-    return HBM_FALLBACK_GBS, "fallback"
+        return float(d["hbm_gbs"]), float(d.get("bf16_tflops_sustained", d.get("bf16_tflops", 1400.0))), "measured"
+    return HBM_FALLBACK_GBS, 1400.0, "fallback"
 
 
 def pick_workload(a) -> W.Workload:
@@ -257,22 +259,28 @@ def run_ours(a):
     value = world * nodes * stages / (ms * 1e-3)
     flops = flops_per_element(w.model, w.N) * w.K
     byts = bytes_per_element(w.model, w.N) * w.K
-    hbm_peak, which = measured_peaks()
+    hbm_peak, bf16_peak, which = measured_peaks()
     t_stage = ms * 1e-3 / stages                          # average stage-kernel duration (copy: <1/(5K) of it)
-    frac_alu = flops / t_stage / (FP32_PEAK_TFLOPS * 1e12)
+    tensor = ctx.variant_name.startswith("tc_")
+    # compute roof of the kernel that ran: FP32 FFMA peak for the SIMT kernel; for the tcgen05 kernels one
+    # fp32-equivalent MAC costs six bf16 MMAs (BF16x3 split) or three tf32 MMAs at half the bf16 rate: bf16 peak / 6
+    comp_peak = bf16_peak / 6.0 if tensor else FP32_PEAK_TFLOPS
+    comp_src = (f"MEASURED_PEAKS.json bf16 sustained ({which}) / 6 (BF16x3 split)" if tensor
+                else "FFMA micro-benchmark, measured (DESIGN.md)")
+    frac_comp = flops / t_stage / (comp_peak * 1e12)
     frac_hbm = byts / t_stage / (hbm_peak * 1e9)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(w.name)
-    if frac_alu >= frac_hbm or flops / (FP32_PEAK_TFLOPS * 1e12) >= byts / (hbm_peak * 1e9):
-        roof = {"bound": "alu", "achieved": flops / t_stage * 1e-12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": frac_alu, "traffic": traffic, "peak_source": "FFMA micro-benchmark, measured (DESIGN.md)",
+        traffic = json.load(open(tpath)).get(w.name + (":tc" if tensor else ":simt"))
+    if flops / (comp_peak * 1e12) >= byts / (hbm_peak * 1e9):      # which roof binds the algorithm on this kernel
+        roof = {"bound": "tensor" if tensor else "alu", "achieved": flops / t_stage * 1e-12, "peak": comp_peak, "unit": "TFLOP/s",
+                "frac": frac_comp, "traffic": traffic, "peak_source": comp_src,
                 "hbm_frac": frac_hbm, "hbm_gbs": byts / t_stage * 1e-9}
     else:
         roof = {"bound": "hbm", "achieved": byts / t_stage * 1e-9, "peak": hbm_peak, "unit": "GB/s", "frac": frac_hbm,
-                "traffic": traffic, "peak_source": f"MEASURED_PEAKS.json ({which})", "alu_frac": frac_alu,
-                "alu_tflops": flops / t_stage * 1e-12}
+                "traffic": traffic, "peak_source": f"MEASURED_PEAKS.json ({which})", "compute_frac": frac_comp,
+                "compute_tflops": flops / t_stage * 1e-12, "compute_peak": comp_peak, "compute_peak_source": comp_src}
     roof["kernel"] = ctx.variant_name
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
@@ -333,7 +341,7 @@ def main():
     ap.add_argument("--sample", type=int, default=None, help="elements in the oracle's timed sample")
     ap.add_argument("--E", type=int, default=0)
     ap.add_argument("--G", type=int, default=0)
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 FP32 SIMT, 2 tensor core (3xTF32), 3 tensor core (BF16x3, warp-specialised)")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 FP32 SIMT, 2 tcgen05 3xTF32, 3 tcgen05 BF16x3 (warp-specialised), 4 tcgen05 BF16x3 (pipelined, every degree)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--sweep", action="store_true")
     a = ap.parse_args()

@@ -69,8 +69,10 @@ typedef struct {              /* HOST, per element, fp64 (piecewise-constant med
 typedef struct {
   int device;                 /* CUDA device ordinal; -1 = host-only context (setup introspection,
                                  no device entry point works: they return DG_ERR_CUDA)           */
-  int variant;                /* 0 = auto; 1 = fused FP32 SIMT stage kernel; 2 = tensor-core (tcgen05,
-                                 3xTF32 split) stage kernel, N <= 7 only (DG_ERR_ARG otherwise)   */
+  int variant;                /* 0 = auto (4 for N >= 2, 1 for N = 1); 1 = fused FP32 SIMT stage kernel;
+                                 2 = tcgen05 3xTF32 kernel, N <= 7; 3 = warp-specialised tcgen05 BF16x3 kernel,
+                                 N <= 7; 4 = pipelined warp-specialised tcgen05 BF16x3 kernel, every degree
+                                 (tensor-core variants need 16-byte aligned q / rhs; DG_ERR_ARG otherwise)  */
   int elems_per_thread;       /* 0 = auto; register blocking E of the SIMT kernel (1..8)         */
   int groups_per_cta;         /* 0 = auto; node groups G per CTA (CTA handles G*E elements)      */
 } dg_options;

@@ -302,7 +302,10 @@ void build_tc3_image(const dgh::RefElem &ref, int NCH, int nsplit, int nstep, st
 }
 
 void choose_variant(dg_ctx *c, const dg_options *o) {
-  const int want = o ? o->variant : 0;
+  int want = o ? o->variant : 0;
+  // auto: the pipelined tensor-core kernel wins from N = 2 up in both models (config-4 sweep);
+  // at N = 1 (Np = 4, three k-steps of padding) the fused SIMT kernel is faster
+  if (want == 0) want = (c->N >= 2 && c->K < (1 << 26)) ? 4 : 1;
   if (want < 0 || want > 4)
     throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core 3xTF32, 3 tensor core BF16x3, 4 pipelined tensor core BF16x3)");
   if (want == 4) {

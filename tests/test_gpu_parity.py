@@ -28,10 +28,14 @@ def _sweep_case(model, N, n=3):
 # ---------------------------------------------------------------- per-RHS parity, every degree, both models
 @pytest.mark.parametrize("N", range(1, 11))
 @pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
-def test_rhs_parity_all_degrees(dg, model, N):
-    """K = 162 elements (several CTAs and a ragged last batch), random N(0,1) fields, random
-    discontinuous materials, free top + rigid walls."""
-    case = Case(dg, _sweep_case(model, N))
+@pytest.mark.parametrize("variant", [1, 4])
+def test_rhs_parity_all_degrees(dg, variant, model, N):
+    """K = 162 elements (several CTAs / batches and a ragged last batch; for the elastic tensor-core
+    kernel with odd Np also batches whose first value is not 16-byte aligned), random N(0,1) fields,
+    random discontinuous materials, free top + rigid walls.  variant 1 = fused FP32 SIMT kernel,
+    variant 4 = pipelined tcgen05 kernel (BF16x3 split, every degree)."""
+    case = Case(dg, _sweep_case(model, N), variant=variant)
+    assert case.ctx.variant_name.startswith("simt_fused" if variant == 1 else "tc_pipe")
     q32 = case.initial_fields32()
     got = case.gpu_rhs(torch, q32)
     want = case.oracle_rhs(q32.astype(np.float64))
@@ -51,11 +55,12 @@ def test_rhs_parity_other_launch_shapes(dg, model, N, E, G):
     assert err <= RHS_TOL, (case.ctx.variant_name, err)
 
 
-def test_rhs_smooth_fields_and_slip_walls(dg):
+@pytest.mark.parametrize("variant", [1, 4])
+def test_rhs_smooth_fields_and_slip_walls(dg, variant):
     """Smooth data (strong cancellation in D q) and the test-only SLIP tag."""
     w = W.config(3, n=3)
     w.top = W.BC_SLIP
-    case = Case(dg, w)
+    case = Case(dg, w, variant=variant)
     q32 = case.initial_fields32()
     assert np.abs(q32).max() > 0.1
     err = rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64)))
@@ -77,10 +82,11 @@ def test_config1_rhs_and_100_steps(dg):
 
 
 # ---------------------------------------------------------------- reduced-size trajectories of configs 2, 3, 5
+@pytest.mark.parametrize("variant", [1, 4])
 @pytest.mark.parametrize("cfg,n", [(2, 6), (3, 4), (5, 2)])
-def test_trajectory_parity_reduced_configs(dg, cfg, n):
+def test_trajectory_parity_reduced_configs(dg, cfg, n, variant):
     w = W.config(cfg, n=n)
-    case = Case(dg, w)
+    case = Case(dg, w, variant=variant)
     q32 = case.initial_fields32()
     dt = case.dt32()
     got = case.gpu_run(torch, q32, dt, w.nsteps)
@@ -125,9 +131,10 @@ def test_full_size_sampled_rhs(dg, cfg):
 
 
 # ---------------------------------------------------------------- API behaviour and edge cases
-def test_edge_cases_and_api_contract(dg):
+@pytest.mark.parametrize("variant", [1, 4])
+def test_edge_cases_and_api_contract(dg, variant):
     w = W.config(1, n=1)                                   # K = 6: less than one batch
-    case = Case(dg, w)
+    case = Case(dg, w, variant=variant)
     ctx = case.ctx
     q32 = case.initial_fields32()
     assert rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64))) <= RHS_TOL
