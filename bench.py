@@ -341,7 +341,7 @@ def main():
     ap.add_argument("--sample", type=int, default=None, help="elements in the oracle's timed sample")
     ap.add_argument("--E", type=int, default=0)
     ap.add_argument("--G", type=int, default=0)
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 FP32 SIMT, 2 tcgen05 3xTF32, 3 tcgen05 BF16x3 (warp-specialised), 4 tcgen05 BF16x3 (pipelined, every degree)")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 fused FP32 SIMT kernel, 4 pipelined tcgen05 BF16x3 kernel")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--sweep", action="store_true")
     a = ap.parse_args()

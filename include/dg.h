@@ -70,9 +70,9 @@ typedef struct {
   int device;                 /* CUDA device ordinal; -1 = host-only context (setup introspection,
                                  no device entry point works: they return DG_ERR_CUDA)           */
   int variant;                /* 0 = auto (4 for N >= 2, 1 for N = 1); 1 = fused FP32 SIMT stage kernel;
-                                 2 = tcgen05 3xTF32 kernel, N <= 7; 3 = warp-specialised tcgen05 BF16x3 kernel,
-                                 N <= 7; 4 = pipelined warp-specialised tcgen05 BF16x3 kernel, every degree
-                                 (tensor-core variants need 16-byte aligned q / rhs; DG_ERR_ARG otherwise)  */
+                                 4 = pipelined warp-specialised tensor-core kernel (tcgen05, BF16x3 split, TMEM
+                                 accumulators), every degree; needs 16-byte aligned q / rhs and K < 2^26.
+                                 Any other value: DG_ERR_ARG                                           */
   int elems_per_thread;       /* 0 = auto; register blocking E of the SIMT kernel (1..8)         */
   int groups_per_cta;         /* 0 = auto; node groups G per CTA (CTA handles G*E elements)      */
 } dg_options;

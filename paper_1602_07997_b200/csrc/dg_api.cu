@@ -13,17 +13,12 @@
 #include "../../include/dg.h"
 #include "host_setup.hpp"
 #include "kernels.cuh"
-#include "tc_kernels.cuh"
-#include "tc2_kernels.cuh"
 #include "tc3_kernels.cuh"
 
 // per-(model, degree) kernel getters from stage_inst.cu
 #define DG_DECL(m, n)                                              \
   extern "C" const void *dgk_get_stage_kernel_##m##_##n(int, int); \
   extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);           \
-  extern "C" const void *dgk_get_tc_kernel_##m##_##n(int);        \
-  extern "C" const void *dgk_get_tc2_kernel_##m##_##n(int);       \
-  extern "C" int dgk_tc2_info_##m##_##n(int);                     \
   extern "C" const void *dgk_get_tc3_kernel_##m##_##n(int);       \
   extern "C" int dgk_tc3_info_##m##_##n(int);
 #define DG_DECL_ALL(m) \
@@ -48,9 +43,6 @@ typedef int (*info_getter)(int);
    fn##m##_10}
 const kernel_getter KERNELS[2][11] = {DG_ROW(0, dgk_get_stage_kernel_), DG_ROW(1, dgk_get_stage_kernel_)};
 const smem_getter SMEM[2][11] = {DG_ROW(0, dgk_stage_smem_bytes_), DG_ROW(1, dgk_stage_smem_bytes_)};
-const tc_getter TC_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc_kernel_), DG_ROW(1, dgk_get_tc_kernel_)};
-const tc_getter TC2_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc2_kernel_), DG_ROW(1, dgk_get_tc2_kernel_)};
-const info_getter TC2_INFO[2][11] = {DG_ROW(0, dgk_tc2_info_), DG_ROW(1, dgk_tc2_info_)};
 const tc_getter TC3_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc3_kernel_), DG_ROW(1, dgk_get_tc3_kernel_)};
 const info_getter TC3_INFO[2][11] = {DG_ROW(0, dgk_tc3_info_), DG_ROW(1, dgk_tc3_info_)};
 
@@ -106,10 +98,8 @@ struct dg_ctx {
   int *d_nbr = nullptr;
   unsigned char *d_fcode = nullptr;
   unsigned short *d_fmask = nullptr, *d_nbrnode = nullptr;
-  float *d_Aimg = nullptr;                       // tensor-core variant 2: operator panel image
-  uint16_t *d_Bimg = nullptr;                    // tensor-core variant 3: bf16x3 operator panel image
-  bool tc2 = false;                              // warp-specialised BF16x3 variant (tc2_kernels.cuh)
-  bool tc3 = false;                              // pipelined BF16x3 variant (tc3_kernels.cuh)
+  uint16_t *d_Bimg = nullptr;                    // tensor-core variant: bf16x3 operator panel image
+  bool tc3 = false;                              // pipelined BF16x3 tensor-core variant (tc3_kernels.cuh)
   int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
@@ -117,7 +107,6 @@ struct dg_ctx {
   const void *k_rhs = nullptr, *k_stage = nullptr;
   int E = 0, G = 0, NT = 0, grid = 0;
   size_t smem = 0;
-  bool tc = false;                               // tensor-core variant (tc_kernels.cuh)
   int nbatch = 0, num_sms = 0;
   int last_launches = 0;
   std::string variant;
@@ -136,7 +125,7 @@ T *upload(const std::vector<T> &h) {
 void free_device(dg_ctx *c) {
   if (c->device < 0) return;
   cudaSetDevice(c->device);
-  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Aimg); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
+  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
 }
@@ -185,46 +174,6 @@ void build_geo_records(const dg_ctx *c, const dg_materials *mat, std::vector<flo
   }
 }
 
-// round to nearest TF32 (ties away, as cvt.rna.tf32.f32): 10 explicit mantissa bits
-float tf32_rn(float x) {
-  uint32_t u;
-  std::memcpy(&u, &x, 4);
-  u = (u + 0x1000u) & 0xFFFFE000u;
-  std::memcpy(&x, &u, 4);
-  return x;
-}
-
-// Operator panel [D_r D_s D_t LIFT] of the tensor-core variant as the shared-memory image the kernel copies
-// verbatim: per stage (3 k-steps of 8) [kstep][hi|lo][k4][128 rows][4] floats, rows >= Np and k beyond the
-// panel are zero.  Node stage g: k-step j = D_j, columns 8g..8g+7; face stage: 24 columns of LIFT.
-// hi = tf32(x), lo = tf32(x - hi) from the fp64 operators (3xTF32 split, tc_kernels.cuh).
-void build_tc_image(const dgh::RefElem &ref, std::vector<float> &img) {
-  const int Np = ref.Np, NFACE = 4 * ref.Nfp;
-  const int NG = (Np + 7) / 8, NFS = (NFACE + 23) / 24;
-  img.assign((size_t)(NG + NFS) * dgk::TC_A_STAGE_FLOATS, 0.f);
-  const std::vector<double> *Dm[3] = {&ref.Dr, &ref.Ds, &ref.Dt};
-  auto put = [&](int st, int ks, int kk, int n, double v) {
-    const float hi = tf32_rn((float)v), lo = tf32_rn((float)(v - (double)hi));
-    const size_t off = (size_t)st * dgk::TC_A_STAGE_FLOATS + (size_t)(ks * 2) * dgk::TC_TILE_FLOATS + (kk >> 2) * 512 + n * 4 + (kk & 3);
-    img[off] = hi;
-    img[off + dgk::TC_TILE_FLOATS] = lo;
-  };
-  for (int st = 0; st < NG; ++st)
-    for (int ks = 0; ks < 3; ++ks)
-      for (int kk = 0; kk < 8; ++kk) {
-        const int m = 8 * st + kk;
-        if (m >= Np) continue;
-        for (int n = 0; n < Np; ++n) put(st, ks, kk, n, (*Dm[ks])[(size_t)n * Np + m]);
-      }
-  for (int fs = 0; fs < NFS; ++fs)
-    for (int ks = 0; ks < 3; ++ks)
-      for (int kk = 0; kk < 8; ++kk) {
-        const int j = fs * 24 + ks * 8 + kk;
-        if (j >= NFACE) continue;
-        for (int n = 0; n < Np; ++n) put(NG + fs, ks, kk, n, ref.LIFT[(size_t)n * NFACE + j]);
-      }
-}
-
 // round to nearest even bf16; returns the 16-bit pattern and the value
 uint16_t bf16_rn(double x, double &val) {
   float f = (float)x;
@@ -236,41 +185,11 @@ uint16_t bf16_rn(double x, double &val) {
   return (uint16_t)(u >> 16);
 }
 
-// Operator panel of variant 3 as the shared-memory image of every k-step (tc2_kernels.cuh):
-// [step][piece 3][kc 2][NC rows n][8 k] bf16, K-major core matrices of 8 rows x 16 bytes.  Step 3g + j holds
-// D_j[n][16g + k], step 3 NG + h holds LIFT[n][16h + k]; entries beyond Np / 4Nfp are zero.  Pieces: BF16x3
-// split of the fp64 operator entry, b1 = bf16(x), b2 = bf16(x - b1), b3 = bf16(x - b1 - b2).
-void build_tc2_image(const dgh::RefElem &ref, int NC, int nstep, std::vector<uint16_t> &img) {
-  const int Np = ref.Np, NFACE = 4 * ref.Nfp;
-  const int NG = (Np + 15) / 16;
-  const size_t stage = (size_t)3 * 2 * NC * 8;
-  img.assign((size_t)nstep * stage, 0);
-  const std::vector<double> *Dm[3] = {&ref.Dr, &ref.Ds, &ref.Dt};
-  auto put = [&](int st, int n, int k, double v) {
-    double v1, v2, v3;
-    const uint16_t b1 = bf16_rn(v, v1), b2 = bf16_rn(v - v1, v2), b3 = bf16_rn(v - v1 - v2, v3);
-    const size_t off = (size_t)st * stage + (size_t)(k >> 3) * NC * 8 + (size_t)n * 8 + (k & 7);
-    img[off] = b1;
-    img[off + (size_t)2 * NC * 8] = b2;
-    img[off + (size_t)4 * NC * 8] = b3;
-  };
-  for (int g = 0; g < NG; ++g)
-    for (int j = 0; j < 3; ++j)
-      for (int k = 0; k < 16; ++k) {
-        const int m = 16 * g + k;
-        if (m >= Np) continue;
-        for (int n = 0; n < Np; ++n) put(3 * g + j, n, k, (*Dm[j])[(size_t)n * Np + m]);
-      }
-  for (int st = 3 * NG; st < nstep; ++st)
-    for (int k = 0; k < 16; ++k) {
-      const int jf = 16 * (st - 3 * NG) + k;
-      if (jf >= NFACE) continue;
-      for (int n = 0; n < Np; ++n) put(st, n, k, ref.LIFT[(size_t)n * NFACE + jf]);
-    }
-}
-
-// Operator panel of variant 4 (tc3_kernels.cuh): as build_tc2_image, but the output nodes are split into NSPLIT
-// contiguous ranges of NCH rows, one image per range: [half][step][piece 3][kc 2][NCH rows n][8 k] bf16.
+// Operator panel of the tensor-core variant as the shared-memory image of every k-step (tc3_kernels.cuh): the output
+// nodes are split into NSPLIT contiguous ranges of NCH rows, one image per range:
+// [half][step][piece 3][kc 2][NCH rows n][8 k] bf16, K-major core matrices of 8 rows x 16 bytes.  Step 3g + j holds
+// D_j[n][16g + k], step 3 NG + h holds LIFT[n][16h + k]; entries beyond Np / 4Nfp are zero.  Pieces: BF16x3 split of
+// the fp64 operator entry, b1 = bf16(x), b2 = bf16(x - b1), b3 = bf16(x - b1 - b2).
 void build_tc3_image(const dgh::RefElem &ref, int NCH, int nsplit, int nstep, std::vector<uint16_t> &img) {
   const int Np = ref.Np, NFACE = 4 * ref.Nfp;
   const int NG = (Np + 15) / 16;
@@ -306,8 +225,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
   // auto: the pipelined tensor-core kernel wins from N = 2 up in both models (config-4 sweep);
   // at N = 1 (Np = 4, three k-steps of padding) the fused SIMT kernel is faster
   if (want == 0) want = (c->N >= 2 && c->K < (1 << 26)) ? 4 : 1;
-  if (want < 0 || want > 4)
-    throw std::invalid_argument("unknown variant (0 auto, 1 SIMT, 2 tensor core 3xTF32, 3 tensor core BF16x3, 4 pipelined tensor core BF16x3)");
+  if (want != 1 && want != 4) throw std::invalid_argument("unknown variant (0 auto, 1 fused FP32 SIMT, 4 pipelined tensor core BF16x3)");
   if (want == 4) {
     if (c->K >= (1 << 26)) throw std::invalid_argument("pipelined tensor-core variant packs the neighbour in 26 bits: K < 2^26");
     c->tc3 = true;
@@ -322,38 +240,6 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     snprintf(buf, sizeof buf, "tc_pipe_bf16x3<%s,N=%d,NCH=%d,nsplit=%d,elems/batch=%d,ksteps=%d,tile=%s x%d,accsets=%d,aring=%d,threads=%d,smem=%zu>",
              c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, info(2), info(4), EB, info(3), info(5) ? "smem" : "L1", info(6), info(7),
              info(8), c->NT, c->smem);
-    c->variant = buf;
-    return;
-  }
-  if (want == 3) {
-    if (!TC2_KERNELS[c->model][c->N](dgk::MODE_STAGE)) throw std::invalid_argument("tensor-core variant needs Np <= 128 (N <= 7)");
-    c->tc2 = true;
-    c->k_rhs = TC2_KERNELS[c->model][c->N](dgk::MODE_RHS);
-    c->k_stage = TC2_KERNELS[c->model][c->N](dgk::MODE_STAGE);
-    const info_getter info = TC2_INFO[c->model][c->N];
-    const int EB = info(1);
-    c->nbatch = (int)((c->K + EB - 1) / EB);
-    c->NT = dgk::T2_THREADS;
-    c->smem = (size_t)info(0);
-    char buf[160];
-    snprintf(buf, sizeof buf, "tc_bf16x3<%s,N=%d,NC=%d,elems/batch=%d,ksteps=%d,threads=%d,smem=%zu>",
-             c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, info(2), EB, info(3), c->NT, c->smem);
-    c->variant = buf;
-    return;
-  }
-  const bool tc_ok = TC_KERNELS[c->model][c->N](dgk::MODE_STAGE) != nullptr;
-  if (want == 2 && !tc_ok) throw std::invalid_argument("tensor-core variant needs Np <= 128 (N <= 7)");
-  c->tc = want == 2;
-  if (c->tc) {
-    c->k_rhs = TC_KERNELS[c->model][c->N](dgk::MODE_RHS);
-    c->k_stage = TC_KERNELS[c->model][c->N](dgk::MODE_STAGE);
-    const int EB = dgk::TC_NCOL / c->NF;
-    c->nbatch = (int)((c->K + EB - 1) / EB);
-    c->NT = dgk::TC_THREADS;
-    c->smem = dgk::TC_SMEM_BYTES;
-    char buf[160];
-    snprintf(buf, sizeof buf, "tc_3xtf32<%s,N=%d,cols=%d,elems/batch=%d,threads=%d,smem=%zu>", c->model == DG_ACOUSTIC ? "acoustic" : "elastic",
-             c->N, dgk::TC_NCOL, EB, c->NT, c->smem);
     c->variant = buf;
     return;
   }
@@ -387,8 +273,6 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   p.DT = c->d_DT; p.LT = c->d_LT; p.geo = c->d_geo; p.nbr = c->d_nbr; p.fcode = c->d_fcode;
   p.fmask = c->d_fmask; p.nbrnode = c->d_nbrnode;
   p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
-  dgk::TcParams tp;
-  dgk::Tc2Params tp2;
   dgk::Tc3Params tp3;
   void *args[] = {&p};
   if (c->tc3) {
@@ -398,20 +282,6 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
     tp3.conn = c->d_conn;
     tp3.nbatch = c->nbatch;
     args[0] = &tp3;
-  }
-  if (c->tc2) {
-    tp2.s = p;
-    tp2.Bimg = c->d_Bimg;
-    tp2.nbatch = c->nbatch;
-    args[0] = &tp2;
-  }
-  if (c->tc) {
-    // the tensor-core kernel reads node quads as float4
-    if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
-    tp.s = p;
-    tp.Aimg = c->d_Aimg;
-    tp.nbatch = c->nbatch;
-    args[0] = &tp;
   }
   cudaError_t e = cudaLaunchKernel(kernel, dim3(c->grid), dim3(c->NT), args, c->smem, st);
   if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " launching " + c->variant);
@@ -493,14 +363,6 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
       c->d_fcode = upload(c->mesh.fcode);
       c->d_fmask = upload(fmask);
       c->d_nbrnode = upload(nbrnode);
-      if (c->tc2) {
-        const info_getter info = TC2_INFO[c->model][c->N];
-        std::vector<uint16_t> img;
-        build_tc2_image(c->ref, info(2), info(3), img);
-        c->d_Bimg = upload(img);
-        CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
-        c->grid = std::min(c->nbatch, c->num_sms);         // persistent: one CTA per SM
-      }
       if (c->tc3) {
         const info_getter info = TC3_INFO[c->model][c->N];
         const int nsplit = info(4);
@@ -513,13 +375,6 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         c->d_conn = upload(conn);
         CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
         c->grid = nsplit * std::max(1, std::min(c->nbatch, c->num_sms / nsplit));   // persistent: one CTA per SM
-      }
-      if (c->tc) {
-        std::vector<float> img;
-        build_tc_image(c->ref, img);
-        c->d_Aimg = upload(img);
-        CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
-        c->grid = std::min(c->nbatch, 2 * c->num_sms);     // persistent: 2 CTAs per SM
       }
       const size_t nq = (size_t)c->K * c->NF * Np;
       CUDA_TRY(cudaMalloc(&c->d_res, nq * sizeof(float)));

@@ -1,8 +1,6 @@
 // One translation unit per (model, degree): compiled with -DDG_MODEL=<0|1> -DDG_N=<1..10>.
 // Exposes the kernel entry points of kernels.cuh for that pair to dg_api.cu through a C getter.
 #include "kernels.cuh"
-#include "tc_kernels.cuh"
-#include "tc2_kernels.cuh"
 #include "tc3_kernels.cuh"
 
 #if !defined(DG_MODEL) || !defined(DG_N)
@@ -36,41 +34,6 @@ extern "C" const void *DG_GETTER(DG_MODEL, DG_N)(int E, int mode) {
 }
 
 extern "C" size_t DG_CAT3(dgk_stage_smem_bytes_, DG_MODEL, DG_N)(int EB) { return dgk::Smem<DG_MODEL, DG_N>::bytes(EB); }
-
-// tensor-core variant (tc_kernels.cuh): one M tile, i.e. Np <= 128 (N <= 7); NULL otherwise
-extern "C" const void *DG_CAT3(dgk_get_tc_kernel_, DG_MODEL, DG_N)(int mode) {
-#if DG_N <= 7
-  if (mode == dgk::MODE_RHS) return (const void *)&dgk::tc_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
-  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::tc_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
-#endif
-  return nullptr;
-}
-
-// warp-specialised BF16x3 tensor-core variant (tc2_kernels.cuh): N <= 7; NULL otherwise
-extern "C" const void *DG_CAT3(dgk_get_tc2_kernel_, DG_MODEL, DG_N)(int mode) {
-#if DG_N <= 7
-  if (mode == dgk::MODE_RHS) return (const void *)&dgk::tc2_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
-  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::tc2_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
-#endif
-  return nullptr;
-}
-// launch geometry of that variant: what = 0 shared-memory bytes, 1 elements per batch, 2 NC, 3 k-steps, 4 bytes per operator stage
-extern "C" int DG_CAT3(dgk_tc2_info_, DG_MODEL, DG_N)(int what) {
-#if DG_N <= 7
-  using C = dgk::T2<DG_MODEL, DG_N>;
-  switch (what) {
-    case 0: return C::SMEM;
-    case 1: return C::EB;
-    case 2: return C::NC;
-    case 3: return C::NSTEP;
-    case 4: return C::BSTAGE;
-    default: return -1;
-  }
-#else
-  (void)what;
-  return -1;
-#endif
-}
 
 // pipelined warp-specialised BF16x3 tensor-core variant (tc3_kernels.cuh): every degree
 extern "C" const void *DG_CAT3(dgk_get_tc3_kernel_, DG_MODEL, DG_N)(int mode) {

@@ -1,6 +1,6 @@
 // Pipelined warp-specialised tensor-core stage kernel of libdg (sm_100a), variant 4: "tc_pipe".
 //
-// Same contraction as tc2_kernels.cuh -- per batch of 32 acoustic / 14 elastic elements (up to 128 (element,
+// One contraction per batch of 32 acoustic / 14 elastic elements (up to 128 (element,
 // field) rows = TMEM lanes)
 //
 //     R[row][n] = sum_k  A[row][k] * B[n][k]
@@ -30,8 +30,7 @@
 
 #include "flux.cuh"
 #include "kernels.cuh"
-#include "tc_kernels.cuh"
-#include "tc2_kernels.cuh"
+#include "tc_common.cuh"
 
 namespace dgk {
 
