@@ -1,10 +1,13 @@
 // libdg C ABI (include/dg.h): context, host setup -> device upload, kernel dispatch.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <array>
 #include <new>
 #include <stdexcept>
 #include <string>
@@ -101,6 +104,9 @@ struct dg_ctx {
   uint16_t *d_Bimg = nullptr;                    // tensor-core variant: bf16x3 operator panel image
   bool tc3 = false;                              // pipelined BF16x3 tensor-core variant (tc3_kernels.cuh)
   int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
+  bool tma_epi = false;                          // tc3: epilogue moves chunks with 2-D TMA (Np % 4 == 0)
+  int epi_cw = 0;                                // tc3: epilogue chunk width (box columns)
+  std::map<const void *, std::array<CUtensorMap, 2>> tmaps;   // device array -> descriptors (box heights 32 / Nf EB - 96)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
   // launch configuration
@@ -236,10 +242,12 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     c->nbatch = (int)((c->K + EB - 1) / EB);
     c->NT = dgk::T3_THREADS;
     c->smem = (size_t)info(0);
-    char buf[200];
-    snprintf(buf, sizeof buf, "tc_pipe_bf16x3<%s,N=%d,NCH=%d,nsplit=%d,elems/batch=%d,ksteps=%d,tile=%s x%d,accsets=%d,aring=%d,threads=%d,smem=%zu>",
+    c->tma_epi = info(10) != 0;
+    c->epi_cw = info(9);
+    char buf[240];
+    snprintf(buf, sizeof buf, "tc_pipe_bf16x3<%s,N=%d,NCH=%d,nsplit=%d,elems/batch=%d,ksteps=%d,tile=%s x%d,accsets=%d,aring=%d,epilogue=%s,threads=%d,smem=%zu>",
              c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, info(2), info(4), EB, info(3), info(5) ? "smem" : "L1", info(6), info(7),
-             info(8), c->NT, c->smem);
+             info(8), info(10) ? "tma" : "cp.async", c->NT, c->smem);
     c->variant = buf;
     return;
   }
@@ -266,6 +274,39 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
   c->variant = buf;
 }
 
+// 2-D TMA descriptors of a [K Nf][Np] fp32 device array for the tensor-core kernel's epilogue: boxes of `epi_cw`
+// nodes x 32 rows ([0]) and x (Nf EB - 96) rows ([1]), 128 B / 64 B swizzle (tc3_kernels.cuh, epilogue)
+typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                    const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+const std::array<CUtensorMap, 2> &tensor_maps(dg_ctx *c, const void *ptr) {
+  auto it = c->tmaps.find(ptr);
+  if (it != c->tmaps.end()) return it->second;
+  static encode_tiled_fn encode = nullptr;
+  if (!encode) {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn)
+      throw std::runtime_error("cuda: cuTensorMapEncodeTiled is not available");
+    encode = (encode_tiled_fn)fn;
+  }
+  if (c->tmaps.size() > 32) c->tmaps.clear();
+  std::array<CUtensorMap, 2> m;
+  const int EB = TC3_INFO[c->model][c->N](1);
+  const int rlast = c->NF * EB - 96;
+  for (int h = 0; h < 2; ++h) {
+    const cuuint64_t dims[2] = {(cuuint64_t)c->Np, (cuuint64_t)c->K * c->NF};
+    const cuuint64_t strides[1] = {(cuuint64_t)c->Np * 4};
+    const cuuint32_t box[2] = {(cuuint32_t)c->epi_cw, (cuuint32_t)(h ? rlast : 32)};
+    const cuuint32_t es[2] = {1, 1};
+    const CUresult r = encode(&m[h], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(ptr), dims, strides, box, es,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, c->epi_cw == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) throw std::runtime_error("cuda: cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+  }
+  return c->tmaps.emplace(ptr, m).first->second;
+}
+
 int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out, float *rhs, float a, float b, float dt,
                  cudaStream_t st) {
   dgk::StageParams p;
@@ -281,6 +322,14 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
     tp3.Bimg = c->d_Bimg;
     tp3.conn = c->d_conn;
     tp3.nbatch = c->nbatch;
+    if (c->tma_epi) {
+      try {
+        const auto &mi = tensor_maps(c, q_in), &mr = tensor_maps(c, c->d_res), &mo = tensor_maps(c, q_out ? q_out : rhs);
+        for (int h = 0; h < 2; ++h) { tp3.tm_in[h] = mi[h]; tp3.tm_res[h] = mr[h]; tp3.tm_out[h] = mo[h]; }
+      } catch (const std::exception &e) {
+        return fail(DG_ERR_CUDA, e.what());
+      }
+    }
     args[0] = &tp3;
   }
   cudaError_t e = cudaLaunchKernel(kernel, dim3(c->grid), dim3(c->NT), args, c->smem, st);

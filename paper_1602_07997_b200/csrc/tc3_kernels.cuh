@@ -25,6 +25,7 @@
 // Warp roles (736 threads): 0-3 epilogue, 4-11 producers (lane = row; tcgen05.st into the TMEM A ring),
 // 12-19 flux, 20 operator stream (cp.async.bulk ring), 21 MMA issue + TMEM allocation, 22 tile loader.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -67,8 +68,9 @@ struct T3 {
   static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
   static constexpr int CW = NC >= 128 ? 16 : 32;               // epilogue chunk width (output nodes)
   static constexpr int SCR = 4 * 4 * 32 * (CW + 4) * 4;        // per epilogue warp: [stage 2][res | q][32][CW + 4] floats
-  static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4;
-  static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 128;
+  static constexpr bool BULK = (NP % 4) == 0;                  // rows are 16-byte aligned: the epilogue moves chunks with TMA
+  static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4 + 8;
+  static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 1024;
   static constexpr int TILE_SLOT = (TILE_RAW + 15) / 16 * 16 + 16;       // + room for a misaligned start
   static constexpr bool TILE = FIXED + TILE_SLOT + META <= T3_SMEM_LIMIT;   // field tile staged in shared memory
   static constexpr int NQ = !TILE ? 2 : (FIXED + 2 * (TILE_SLOT + META) <= T3_SMEM_LIMIT ? 2 : 1);
@@ -79,7 +81,7 @@ struct T3 {
   static constexpr int OFF_SCR = OFF_FLUX + T3_NFL * FLUX_SLOT;
   static constexpr int OFF_SLOT = OFF_SCR + SCR;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
-  static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 128;   // + slack for the 128-byte alignment
+  static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 1024;  // + slack for the 1024-byte alignment (swizzled TMA boxes)
   static constexpr int TPT = (EB * 16 + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
   static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
   static_assert(NA >= 3, "A ring too small");
@@ -116,6 +118,9 @@ struct Tc3Params {
   const uint16_t *__restrict__ Bimg;   // [NSPLIT][NSTEP][3][2][NCH][8] bf16 operator panel image (host: build_tc3_image)
   const int *__restrict__ conn;        // [K][4] packed connectivity: (neighbour << 5 | face code) or -(bc tag)
   int nbatch;
+  // epilogue TMA descriptors (only when Np % 4 == 0): 2-D views [K Nf rows][Np] of q_in, res and q_out | rhs with
+  // boxes of CW nodes x 32 rows ([0]) and CW x (Nf EB - 96) rows ([1], the last row quadrant of an elastic batch)
+  CUtensorMap tm_in[2], tm_res[2], tm_out[2];
 };
 
 namespace tc {
@@ -147,6 +152,19 @@ __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t *v) {
         : "memory");
   }
 }
+// 2-D tiled TMA: global -> shared (completion on an mbarrier) and shared -> global (bulk async-group)
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int x, int y, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+               "l"(map), "r"(x), "r"(y), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, int x, int y, uint32_t src) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];" ::"l"(map), "r"(x), "r"(y), "r"(src)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void *src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
 }
@@ -211,7 +229,7 @@ __device__ __forceinline__ void row_coefficients_s(const float *g, int f, float 
 
 // ---- the kernel ------------------------------------------------------------------------------------
 template <int MODEL, int N, int MODE>
-__global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Params P) {
+__global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_constant__ Tc3Params P) {
   using C = T3<MODEL, N>;
   constexpr int NP = C::NP, NFP = C::NFP, NFACE = C::NFACE, NF = C::NF, NGEO = C::NGEO, EB = C::EB, NCH = C::NCH;
   constexpr int NA = C::NA, NB = T3_NB, NFL = T3_NFL, NQ = C::NQ;
@@ -219,7 +237,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
   const StageParams &p = P.s;
 
   extern __shared__ unsigned char smem_raw[];
-  unsigned char *sm = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+  unsigned char *sm = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   unsigned char *sB = sm + C::OFF_B;                               // [NB][3][2][NCH][8] bf16
   float *s_flux = reinterpret_cast<float *>(sm + C::OFF_FLUX);     // [NFL][128][FLS] penalty-term chunks
   float *s_scr = reinterpret_cast<float *>(sm + C::OFF_SCR);       // epilogue staging (see the epilogue)
@@ -242,6 +260,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
   auto accEmpty = [&](int t) { return barX + 8u * (2 + t); };
   auto qFull = [&](int t) { return barX + 8u * (4 + t); };
   auto qEmpty = [&](int t) { return barX + 8u * (6 + t); };
+  auto epiFull = [&](int w, int t) { return barX + 8u * (8 + 2 * w + t); };
   // byte offset of the batch's first field value inside its tile slot (bulk copies start 16-byte aligned)
   auto tile_shift = [&](int k0) { return (uint32_t)(((size_t)k0 * NF * NP * 4) & 15); };
 
@@ -256,6 +275,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
     for (int t = 0; t < 2; ++t) {
       tc::mbar_init(accFull(t), 1); tc::mbar_init(accEmpty(t), 4);
       tc::mbar_init(qFull(t), 1); tc::mbar_init(qEmpty(t), 8 + T3_FLUXW);
+      for (int w = 0; w < 4; ++w) tc::mbar_init(epiFull(w, t), 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -269,6 +289,102 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
 #endif
 
   if (warp < 4) {
+    if constexpr (C::BULK) {
+    // =================================================== epilogue: LSRK update (row a7), TMA path (Np % 4 == 0)
+    // Chunks of 32 rows x CW output nodes move as 2-D TMA boxes: res / q in two chunks ahead (mbarrier per warp
+    // and stage), results out through the same swizzled staging buffers (bulk async-group).  The update runs in
+    // the TMEM-native layout (thread = row); the 128 B / 64 B swizzle keeps its float4 accesses conflict-free.
+    constexpr int CW = C::CW;
+    constexpr uint32_t BUFB = 32 * CW * 4;             // bytes of one staging buffer (1024-byte aligned)
+    constexpr int RLAST = C::NR - 96;                  // rows of the last quadrant (32 acoustic, 30 elastic)
+    const int qd = warp;
+    const int hmap = (qd == 3 && RLAST != 32) ? 1 : 0; // which box height
+    const uint32_t boxbytes = (uint32_t)((hmap ? RLAST : 32) * CW * 4);
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(s_scr) + warp * (4 * BUFB);   // [stage 2][res | q]
+    const int n0 = hid * NCH;
+    const int ncv = min(NCH, NP - n0);
+    const bool need_res = MODE == MODE_STAGE && p.a != 0.f;
+    const bool leader = tc::elect_one();               // the same lane issues and retires every TMA operation
+    auto issue = [&](int stg, int b, int c0) {         // TMA loads of chunk (b, c0) into stage stg
+      if (MODE == MODE_STAGE && b < P.nbatch && leader) {
+        const int row0 = b * EB * NF + qd * 32;
+        const uint32_t dR = tc::smem_u32(bufs + (stg * 2) * BUFB), dQ = dR + BUFB;
+        tc::mbar_expect_tx(epiFull(warp, stg), need_res ? 2 * boxbytes : boxbytes);
+        tc::tma_load_2d(dQ, &P.tm_in[hmap], n0 + c0, row0, epiFull(warp, stg));
+        if (need_res) tc::tma_load_2d(dR, &P.tm_res[hmap], n0 + c0, row0, epiFull(warp, stg));
+      }
+    };
+    auto advance = [&](int &b, int &c0) {
+      c0 += CW;
+      if (c0 >= ncv) { c0 = 0; b += nworkers; }
+    };
+    int ab = worker, ac0 = 0;                          // the chunk two ahead of the current one
+    issue(0, ab, ac0);
+    advance(ab, ac0);
+    issue(1, ab, ac0);
+    advance(ab, ac0);
+    int it = -1, stg = 0, set = 0;
+    uint32_t par[2] = {0, 0};
+    for (int b = worker, c0 = 0; b < P.nbatch; advance(b, c0), stg ^= 1) {
+      if (c0 == 0) {
+        ++it;
+        set = C::NSETS == 2 ? (it & 1) : 0;
+        T3_WAIT(accFull(set), (C::NSETS == 2 ? (it >> 1) : it) & 1, 0);
+        tc::tc_fence_after();
+      }
+      const uint32_t t0 = tm + ((uint32_t)(qd * 32) << 16) + set * 2 * NCH + c0;
+      uint32_t vm[CW], vs[CW];
+      T3_TIMED(2, tc::tmem_ld<CW>(t0, vm); tc::tmem_ld<CW>(t0 + NCH, vs));
+      if (c0 + CW >= ncv) {              // accumulators drained: the MMA warp may start the next batch on this set
+        tc::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) tc::mbar_arrive(accEmpty(set));
+      }
+      if (MODE == MODE_STAGE) {
+        T3_WAIT(epiFull(warp, stg), par[stg], 1);      // this chunk's boxes have landed
+        par[stg] ^= 1;
+      }
+      unsigned char *bR = bufs + (stg * 2) * BUFB, *bQ = bR + BUFB;
+      // swizzle: 16-byte chunk j4 of row `lane` sits at chunk j4 ^ f(lane) (128B: lane & 7, 64B: (lane >> 1) & 3)
+      const int sw = CW == 32 ? (lane & 7) : ((lane >> 1) & 3);
+#pragma unroll
+      for (int j4 = 0; j4 < CW / 4; ++j4) {
+        const int off = lane * (CW * 4) + ((j4 ^ sw) << 4);
+        float4 *pr = reinterpret_cast<float4 *>(bR + off), *pq = reinterpret_cast<float4 *>(bQ + off);
+        float r[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) r[t] = __uint_as_float(vm[4 * j4 + t]) + __uint_as_float(vs[4 * j4 + t]);
+        if (MODE == MODE_RHS) {
+          *pr = make_float4(r[0], r[1], r[2], r[3]);
+        } else {
+          float4 R = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (need_res) R = *pr;
+          const float4 Q = *pq;
+          R.x = fmaf(p.a, R.x, p.dt * r[0]); R.y = fmaf(p.a, R.y, p.dt * r[1]);
+          R.z = fmaf(p.a, R.z, p.dt * r[2]); R.w = fmaf(p.a, R.w, p.dt * r[3]);
+          *pr = R;
+          *pq = make_float4(fmaf(p.b, R.x, Q.x), fmaf(p.b, R.y, Q.y), fmaf(p.b, R.z, Q.z), fmaf(p.b, R.w, Q.w));
+        }
+      }
+      tc::fence_proxy_async();           // generic-proxy writes -> visible to the TMA store
+      __syncwarp();
+      if (leader) {
+        const int row0 = b * EB * NF + qd * 32;
+        if (MODE == MODE_RHS) {
+          tc::tma_store_2d(&P.tm_out[hmap], n0 + c0, row0, tc::smem_u32(bR));
+        } else {
+          tc::tma_store_2d(&P.tm_res[hmap], n0 + c0, row0, tc::smem_u32(bR));
+          tc::tma_store_2d(&P.tm_out[hmap], n0 + c0, row0, tc::smem_u32(bQ));
+        }
+        tc::bulk_commit();
+        tc::bulk_wait_read0();           // the stores have read the staging buffers: the stage can be refilled
+      }
+      __syncwarp();
+      issue(stg, ab, ac0);
+      advance(ab, ac0);
+    }
+    if (leader) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    } else {
     // =================================================== epilogue: LSRK update (row a7)
     // Chunks of 32 rows x CW output nodes.  The chunk's res / q values are brought into a per-warp staging
     // buffer by cp.async two chunks ahead (no register or scoreboard is held while they are in flight), the
@@ -362,6 +478,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const Tc3Param
       advance(ab, ac0);
     }
     tc::cp_async_wait<0>();
+    }
   } else if (warp < 12) {
     // =================================================== producers: rows a1 + a3, BF16x3 split, tcgen05.st
     const int pw = warp - 4, qd = pw & 3, half = pw >> 2;
