@@ -104,8 +104,9 @@ struct dg_ctx {
   uint16_t *d_Bimg = nullptr;                    // tensor-core variant: bf16x3 operator panel image
   bool tc3 = false;                              // pipelined BF16x3 tensor-core variant (tc3_kernels.cuh)
   int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
-  bool tma_epi = false;                          // tc3: epilogue moves chunks with 2-D TMA (Np % 4 == 0)
-  int epi_cw = 0;                                // tc3: epilogue chunk width (box columns)
+  int epi_cw = 0;                                // tc3: epilogue chunk width (TMA box columns)
+  int PT = 0;                                    // tc3: row pitch (floats) of the arrays the kernel works on, Np rounded up to 4
+  float *d_qa = nullptr;                         // tc3, PT != Np: padded private copies of the state (d_qa and d_q2 ping-pong)
   std::map<const void *, std::array<CUtensorMap, 2>> tmaps;   // device array -> descriptors (box heights 32 / Nf EB - 96)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
@@ -131,7 +132,7 @@ T *upload(const std::vector<T> &h) {
 void free_device(dg_ctx *c) {
   if (c->device < 0) return;
   cudaSetDevice(c->device);
-  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
+  cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_qa); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
 }
@@ -228,9 +229,9 @@ void build_tc3_image(const dgh::RefElem &ref, int NCH, int nsplit, int nstep, st
 
 void choose_variant(dg_ctx *c, const dg_options *o) {
   int want = o ? o->variant : 0;
-  // auto: the pipelined tensor-core kernel wins from N = 2 up in both models (config-4 sweep);
-  // at N = 1 (Np = 4, three k-steps of padding) the fused SIMT kernel is faster
-  if (want == 0) want = (c->N >= 2 && c->K < (1 << 26)) ? 4 : 1;
+  // auto: the tensor-core kernel wins everywhere in the config-4 sweep except elastic N = 1
+  // (Np = 4: three of four k-steps are padding), where the fused SIMT kernel is faster
+  if (want == 0) want = ((c->N >= 2 || c->model == DG_ACOUSTIC) && c->K < (1 << 26)) ? 4 : 1;
   if (want != 1 && want != 4) throw std::invalid_argument("unknown variant (0 auto, 1 fused FP32 SIMT, 4 pipelined tensor core BF16x3)");
   if (want == 4) {
     if (c->K >= (1 << 26)) throw std::invalid_argument("pipelined tensor-core variant packs the neighbour in 26 bits: K < 2^26");
@@ -242,12 +243,12 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     c->nbatch = (int)((c->K + EB - 1) / EB);
     c->NT = dgk::T3_THREADS;
     c->smem = (size_t)info(0);
-    c->tma_epi = info(10) != 0;
     c->epi_cw = info(9);
+    c->PT = info(10);
     char buf[240];
-    snprintf(buf, sizeof buf, "tc_pipe_bf16x3<%s,N=%d,NCH=%d,nsplit=%d,elems/batch=%d,ksteps=%d,tile=%s x%d,accsets=%d,aring=%d,epilogue=%s,threads=%d,smem=%zu>",
+    snprintf(buf, sizeof buf, "tc_pipe_bf16x3<%s,N=%d,NCH=%d,nsplit=%d,elems/batch=%d,ksteps=%d,tile=%s x%d,accsets=%d,aring=%d,pitch=%d,threads=%d,smem=%zu>",
              c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, info(2), info(4), EB, info(3), info(5) ? "smem" : "L1", info(6), info(7),
-             info(8), info(10) ? "tma" : "cp.async", c->NT, c->smem);
+             info(8), info(10), c->NT, c->smem);
     c->variant = buf;
     return;
   }
@@ -274,7 +275,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
   c->variant = buf;
 }
 
-// 2-D TMA descriptors of a [K Nf][Np] fp32 device array for the tensor-core kernel's epilogue: boxes of `epi_cw`
+// 2-D TMA descriptors of a [K Nf][PT] fp32 device array for the tensor-core kernel's epilogue: boxes of `epi_cw`
 // nodes x 32 rows ([0]) and x (Nf EB - 96) rows ([1]), 128 B / 64 B swizzle (tc3_kernels.cuh, epilogue)
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -295,8 +296,8 @@ const std::array<CUtensorMap, 2> &tensor_maps(dg_ctx *c, const void *ptr) {
   const int EB = TC3_INFO[c->model][c->N](1);
   const int rlast = c->NF * EB - 96;
   for (int h = 0; h < 2; ++h) {
-    const cuuint64_t dims[2] = {(cuuint64_t)c->Np, (cuuint64_t)c->K * c->NF};
-    const cuuint64_t strides[1] = {(cuuint64_t)c->Np * 4};
+    const cuuint64_t dims[2] = {(cuuint64_t)c->PT, (cuuint64_t)c->K * c->NF};
+    const cuuint64_t strides[1] = {(cuuint64_t)c->PT * 4};
     const cuuint32_t box[2] = {(cuuint32_t)c->epi_cw, (cuuint32_t)(h ? rlast : 32)};
     const cuuint32_t es[2] = {1, 1};
     const CUresult r = encode(&m[h], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(ptr), dims, strides, box, es,
@@ -322,7 +323,7 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
     tp3.Bimg = c->d_Bimg;
     tp3.conn = c->d_conn;
     tp3.nbatch = c->nbatch;
-    if (c->tma_epi) {
+    {
       try {
         const auto &mi = tensor_maps(c, q_in), &mr = tensor_maps(c, c->d_res), &mo = tensor_maps(c, q_out ? q_out : rhs);
         for (int h = 0; h < 2; ++h) { tp3.tm_in[h] = mi[h]; tp3.tm_res[h] = mr[h]; tp3.tm_out[h] = mo[h]; }
@@ -426,13 +427,21 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         c->grid = nsplit * std::max(1, std::min(c->nbatch, c->num_sms / nsplit));   // persistent: one CTA per SM
       }
       const size_t nq = (size_t)c->K * c->NF * Np;
-      CUDA_TRY(cudaMalloc(&c->d_res, nq * sizeof(float)));
-      CUDA_TRY(cudaMalloc(&c->d_q2, nq * sizeof(float)));
+      // the tensor-core kernel works on rows of pitch PT (16-byte aligned); when PT != Np the state lives in padded private
+      // copies (pad columns are zero and stay zero) and is converted on entry / exit of every API call
+      const size_t nqp = c->tc3 ? (size_t)c->K * c->NF * c->PT : nq;
+      CUDA_TRY(cudaMalloc(&c->d_res, nqp * sizeof(float)));
+      CUDA_TRY(cudaMalloc(&c->d_q2, nqp * sizeof(float)));
+      CUDA_TRY(cudaMemset(c->d_q2, 0, nqp * sizeof(float)));
+      if (c->tc3 && c->PT != Np) {
+        CUDA_TRY(cudaMalloc(&c->d_qa, nqp * sizeof(float)));
+        CUDA_TRY(cudaMemset(c->d_qa, 0, nqp * sizeof(float)));
+      }
       for (float *&h : c->d_hist) {
         CUDA_TRY(cudaMalloc(&h, nq * sizeof(float)));
         CUDA_TRY(cudaMemset(h, 0, nq * sizeof(float)));
       }
-      CUDA_TRY(cudaMemset(c->d_res, 0, nq * sizeof(float)));
+      CUDA_TRY(cudaMemset(c->d_res, 0, nqp * sizeof(float)));
       CUDA_TRY(cudaFuncSetAttribute(c->k_rhs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
       CUDA_TRY(cudaFuncSetAttribute(c->k_stage, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
       CUDA_TRY(cudaDeviceSynchronize());
@@ -544,20 +553,56 @@ int dg_connectivity(const dg_ctx *c, int32_t *elemP, int32_t *nodeP, int8_t *bct
   return DG_OK;
 }
 
+// caller layout [K Nf][Np] <-> the tensor-core kernel's private layout [K Nf][PT] (pad columns stay zero)
+static bool padded(const dg_ctx *c) { return c->tc3 && c->PT != c->Np; }
+static int copy_rows(dg_ctx *c, float *dst, int dpitch, const float *src, int spitch, cudaStream_t st) {
+  cudaError_t e = cudaMemcpy2DAsync(dst, (size_t)dpitch * 4, src, (size_t)spitch * 4, (size_t)c->Np * 4, (size_t)c->K * c->NF,
+                                    cudaMemcpyDeviceToDevice, st);
+  if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " in the layout conversion");
+  return DG_OK;
+}
+// r(q) -> d_out (caller layout); adds the number of launches / copies enqueued to `launches`
+static int eval_rhs(dg_ctx *c, const float *d_q, float *d_out, cudaStream_t st, int &launches) {
+  if (!padded(c)) {
+    launches += 1;
+    return launch_stage(c, c->k_rhs, d_q, nullptr, d_out, 0.f, 0.f, 0.f, st);
+  }
+  if (int e = copy_rows(c, c->d_qa, c->PT, d_q, c->Np, st)) return e;
+  if (int e = launch_stage(c, c->k_rhs, c->d_qa, nullptr, c->d_q2, 0.f, 0.f, 0.f, st)) return e;
+  launches += 3;
+  return copy_rows(c, d_out, c->Np, c->d_q2, c->PT, st);
+}
+
 int dg_rhs(dg_ctx *c, const float *d_q, float *d_rhs, void *stream) {
   if (int e = check_device_ctx(c)) return e;
   if (!d_q || !d_rhs) return fail(DG_ERR_ARG, "NULL device pointer");
   if (d_q == d_rhs) return fail(DG_ERR_ARG, "dg_rhs: d_q and d_rhs must differ");
-  c->last_launches = 1;
-  return launch_stage(c, c->k_rhs, d_q, nullptr, d_rhs, 0.f, 0.f, 0.f, (cudaStream_t)stream);
+  c->last_launches = 0;
+  return eval_rhs(c, d_q, d_rhs, (cudaStream_t)stream, c->last_launches);
 }
 
 int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
   if (int e = check_device_ctx(c)) return e;
   if (!d_q || nsteps < 0) return fail(DG_ERR_ARG, "bad argument");
   cudaStream_t st = (cudaStream_t)stream;
-  float *cur = d_q, *oth = c->d_q2;
   int launches = 0;
+  if (padded(c)) {
+    // private padded state: convert once on entry and once on exit, the 5 nsteps stage kernels ping-pong d_qa <-> d_q2
+    if (nsteps > 0) {
+      if (int e = copy_rows(c, c->d_qa, c->PT, d_q, c->Np, st)) return e;
+      float *cur = c->d_qa, *oth = c->d_q2;
+      for (int s = 0; s < nsteps; ++s)
+        for (int i = 0; i < 5; ++i) {
+          if (int e = launch_stage(c, c->k_stage, cur, oth, nullptr, (float)RK_A[i], (float)RK_B[i], dt, st)) return e;
+          std::swap(cur, oth);
+        }
+      if (int e = copy_rows(c, d_q, c->Np, cur, c->PT, st)) return e;
+      launches = 5 * nsteps + 2;
+    }
+    c->last_launches = launches;
+    return DG_OK;
+  }
+  float *cur = d_q, *oth = c->d_q2;
   for (int s = 0; s < nsteps; ++s)
     for (int i = 0; i < 5; ++i) {
       if (int e = launch_stage(c, c->k_stage, cur, oth, nullptr, (float)RK_A[i], (float)RK_B[i], dt, st)) return e;
@@ -591,10 +636,10 @@ int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) {
   // rotate history: r0 <- new, r1, r2 older (Table 1: R_0, R_-1, R_-2)
   c->hist_head = (c->hist_head + 2) % 3;
   float *r0 = c->d_hist[c->hist_head], *r1 = c->d_hist[(c->hist_head + 1) % 3], *r2 = c->d_hist[(c->hist_head + 2) % 3];
-  if (int e = launch_stage(c, c->k_rhs, d_q, nullptr, r0, 0.f, 0.f, 0.f, st)) return e;
+  int launches = 0;
+  if (int e = eval_rhs(c, d_q, r0, st, launches)) return e;
   const size_t nq = (size_t)c->K * c->NF * c->Np, n4 = nq / 4;
   const float c0 = dt * (23.f / 12.f), c1 = dt * (-16.f / 12.f), c2 = dt * (5.f / 12.f);
-  int launches = 1;
   if (n4) {
     const int blocks = (int)std::min<size_t>((n4 + 255) / 256, (size_t)148 * 16);
     dgk::ab3_update_kernel<<<blocks, 256, 0, st>>>((float4 *)d_q, (const float4 *)r0, (const float4 *)r1, (const float4 *)r2, n4, c0, c1, c2);

@@ -42,7 +42,7 @@ extern "C" const void *DG_CAT3(dgk_get_tc3_kernel_, DG_MODEL, DG_N)(int mode) {
   return nullptr;
 }
 // launch geometry: what = 0 shared-memory bytes, 1 elements per batch, 2 NCH, 3 k-steps, 4 NSPLIT, 5 tile staged in
-// shared memory, 6 tile slots, 7 accumulator sets, 8 A ring stages, 9 epilogue chunk width, 10 TMA epilogue
+// shared memory, 6 tile slots, 7 accumulator sets, 8 A ring stages, 9 epilogue chunk width, 10 row pitch of q / res / rhs (floats)
 extern "C" int DG_CAT3(dgk_tc3_info_, DG_MODEL, DG_N)(int what) {
   using C = dgk::T3<DG_MODEL, DG_N>;
   switch (what) {
@@ -56,7 +56,7 @@ extern "C" int DG_CAT3(dgk_tc3_info_, DG_MODEL, DG_N)(int what) {
     case 7: return C::NSETS;
     case 8: return C::NA;
     case 9: return C::CW;
-    case 10: return C::BULK ? 1 : 0;
+    case 10: return C::PT;
     default: return -1;
   }
 }

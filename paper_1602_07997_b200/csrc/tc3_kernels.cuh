@@ -52,6 +52,7 @@ struct T3 {
   static constexpr int NGEO = MODEL == 0 ? GEO_AC : GEO_EL;
   static constexpr int EB = MODEL == 0 ? 32 : 14;              // elements per batch
   static constexpr int NR = EB * NF;                           // valid rows (<= 128)
+  static constexpr int PT = (NP + 3) / 4 * 4;                  // row pitch of q / res / rhs (floats): rows 16-byte aligned
   static constexpr int NC = (NP + 15) / 16 * 16;               // output nodes, padded
   static constexpr int NSPLIT = NC > 176 ? 2 : 1;              // CTAs sharing one batch (output-node halves)
   static constexpr int NCH = NC / NSPLIT;                      // MMA N of one CTA
@@ -63,15 +64,14 @@ struct T3 {
   static constexpr int NA_ = (512 - ABASE) / T3_ASTRIDE;
   static constexpr int NA = NA_ > 9 ? 9 : NA_;                 // A ring stages
   static constexpr int BSTAGE = 96 * NCH;                      // bytes: [3 pieces][2 kc][NCH][8] bf16
-  static constexpr int TILE_RAW = EB * NF * NP * 4;            // bytes of the batch's fields
+  static constexpr int TILE_RAW = EB * NF * PT * 4;            // bytes of the batch's fields (multiple of 16)
   static constexpr int META = EB * NGEO * 4 + EB * 16;         // geometric records + packed connectivity
   static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
   static constexpr int CW = NC >= 128 ? 16 : 32;               // epilogue chunk width (output nodes)
   static constexpr int SCR = 4 * 4 * 32 * (CW + 4) * 4;        // per epilogue warp: [stage 2][res | q][32][CW + 4] floats
-  static constexpr bool BULK = (NP % 4) == 0;                  // rows are 16-byte aligned: the epilogue moves chunks with TMA
   static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4 + 8;
   static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 1024;
-  static constexpr int TILE_SLOT = (TILE_RAW + 15) / 16 * 16 + 16;       // + room for a misaligned start
+  static constexpr int TILE_SLOT = TILE_RAW;
   static constexpr bool TILE = FIXED + TILE_SLOT + META <= T3_SMEM_LIMIT;   // field tile staged in shared memory
   static constexpr int NQ = !TILE ? 2 : (FIXED + 2 * (TILE_SLOT + META) <= T3_SMEM_LIMIT ? 2 : 1);
   static constexpr int SLOT = (TILE ? TILE_SLOT : 0) + META;   // bytes of one tile slot
@@ -118,7 +118,7 @@ struct Tc3Params {
   const uint16_t *__restrict__ Bimg;   // [NSPLIT][NSTEP][3][2][NCH][8] bf16 operator panel image (host: build_tc3_image)
   const int *__restrict__ conn;        // [K][4] packed connectivity: (neighbour << 5 | face code) or -(bc tag)
   int nbatch;
-  // epilogue TMA descriptors (only when Np % 4 == 0): 2-D views [K Nf rows][Np] of q_in, res and q_out | rhs with
+  // epilogue TMA descriptors: 2-D views [K Nf rows][PT] of q_in, res and q_out | rhs with
   // boxes of CW nodes x 32 rows ([0]) and CW x (Nf EB - 96) rows ([1], the last row quadrant of an elastic batch)
   CUtensorMap tm_in[2], tm_res[2], tm_out[2];
 };
@@ -231,7 +231,7 @@ __device__ __forceinline__ void row_coefficients_s(const float *g, int f, float 
 template <int MODEL, int N, int MODE>
 __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_constant__ Tc3Params P) {
   using C = T3<MODEL, N>;
-  constexpr int NP = C::NP, NFP = C::NFP, NFACE = C::NFACE, NF = C::NF, NGEO = C::NGEO, EB = C::EB, NCH = C::NCH;
+  constexpr int NP = C::NP, PT = C::PT, NFP = C::NFP, NFACE = C::NFACE, NF = C::NF, NGEO = C::NGEO, EB = C::EB, NCH = C::NCH;
   constexpr int NA = C::NA, NB = T3_NB, NFL = T3_NFL, NQ = C::NQ;
   constexpr bool TILE = C::TILE;
   const StageParams &p = P.s;
@@ -261,8 +261,6 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
   auto qFull = [&](int t) { return barX + 8u * (4 + t); };
   auto qEmpty = [&](int t) { return barX + 8u * (6 + t); };
   auto epiFull = [&](int w, int t) { return barX + 8u * (8 + 2 * w + t); };
-  // byte offset of the batch's first field value inside its tile slot (bulk copies start 16-byte aligned)
-  auto tile_shift = [&](int k0) { return (uint32_t)(((size_t)k0 * NF * NP * 4) & 15); };
 
   if (warp == T3_W_MMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(s_tmem)), "n"(512) : "memory");
@@ -289,8 +287,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #endif
 
   if (warp < 4) {
-    if constexpr (C::BULK) {
-    // =================================================== epilogue: LSRK update (row a7), TMA path (Np % 4 == 0)
+    // =================================================== epilogue: LSRK update (row a7)
     // Chunks of 32 rows x CW output nodes move as 2-D TMA boxes: res / q in two chunks ahead (mbarrier per warp
     // and stage), results out through the same swizzled staging buffers (bulk async-group).  The update runs in
     // the TMEM-native layout (thread = row); the 128 B / 64 B swizzle keeps its float4 accesses conflict-free.
@@ -384,108 +381,12 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       advance(ab, ac0);
     }
     if (leader) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-    } else {
-    // =================================================== epilogue: LSRK update (row a7)
-    // Chunks of 32 rows x CW output nodes.  The chunk's res / q values are brought into a per-warp staging
-    // buffer by cp.async two chunks ahead (no register or scoreboard is held while they are in flight), the
-    // update runs in the TMEM-native layout (thread = row), the results go back into the same buffer and
-    // leave through coalesced stores (lanes = consecutive nodes of one row).
-    constexpr int CW = C::CW, PITCH = CW + 4, RPI = 32 / CW;
-    const int qd = warp;
-    float *bufs = s_scr + warp * (4 * 32 * PITCH);     // [stage 2][res | q][32 rows][PITCH]
-    const int n0 = hid * NCH;
-    const int ncv = min(NCH, NP - n0);                 // valid output nodes of this CTA
-    const bool need_res = MODE == MODE_STAGE && p.a != 0.f;
-    const int sub = lane / CW, col = lane % CW;        // RPI rows per load / store instruction
-    auto issue = [&](int stg, int b, int c0) {         // async loads of chunk (b, c0) into stage stg
-      if (MODE == MODE_STAGE && b < P.nbatch && c0 + col < ncv) {
-        const int k0 = b * EB;
-        const int rmax = min(32, min(EB, p.K - k0) * NF - qd * 32);
-        const size_t base = ((size_t)k0 * NF + qd * 32) * NP + n0 + c0 + col;
-        const uint32_t dR = tc::smem_u32(bufs + (stg * 2) * 32 * PITCH + col), dQ = dR + 32 * PITCH * 4;
-#pragma unroll 4
-        for (int rr = sub; rr < rmax; rr += RPI) {
-          tc::cp_async4(dQ + rr * PITCH * 4, p.q_in + base + (size_t)rr * NP);
-          if (need_res) tc::cp_async4(dR + rr * PITCH * 4, p.res + base + (size_t)rr * NP);
-        }
-      }
-      tc::cp_async_commit();
-    };
-    auto advance = [&](int &b, int &c0) {
-      c0 += CW;
-      if (c0 >= ncv) { c0 = 0; b += nworkers; }
-    };
-    int ab = worker, ac0 = 0;                          // the chunk two ahead of the current one
-    issue(0, ab, ac0);
-    advance(ab, ac0);
-    issue(1, ab, ac0);
-    advance(ab, ac0);
-    int it = -1, stg = 0, set = 0;
-    for (int b = worker, c0 = 0; b < P.nbatch; advance(b, c0), stg ^= 1) {
-      const int k0 = b * EB;
-      const int rmax = min(32, min(EB, p.K - k0) * NF - qd * 32);
-      if (c0 == 0) {
-        ++it;
-        set = C::NSETS == 2 ? (it & 1) : 0;
-        T3_WAIT(accFull(set), (C::NSETS == 2 ? (it >> 1) : it) & 1, 0);
-        tc::tc_fence_after();
-      }
-      const uint32_t t0 = tm + ((uint32_t)(qd * 32) << 16) + set * 2 * NCH + c0;
-      uint32_t vm[CW], vs[CW];
-      T3_TIMED(2, tc::tmem_ld<CW>(t0, vm); tc::tmem_ld<CW>(t0 + NCH, vs));
-      if (c0 + CW >= ncv) {              // accumulators drained: the MMA warp may start the next batch on this set
-        tc::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) tc::mbar_arrive(accEmpty(set));
-      }
-      T3_TIMED(1, tc::cp_async_wait<1>());   // this chunk's loads have landed (the next chunk's may be in flight)
-      __syncwarp();
-      float *bR = bufs + (stg * 2) * 32 * PITCH, *bQ = bR + 32 * PITCH;
-#pragma unroll
-      for (int j4 = 0; j4 < CW / 4; ++j4) {
-        float4 *pr = reinterpret_cast<float4 *>(bR + lane * PITCH + 4 * j4), *pq = reinterpret_cast<float4 *>(bQ + lane * PITCH + 4 * j4);
-        float r[4];
-#pragma unroll
-        for (int t = 0; t < 4; ++t) r[t] = __uint_as_float(vm[4 * j4 + t]) + __uint_as_float(vs[4 * j4 + t]);
-        if (MODE == MODE_RHS) {
-          *pr = make_float4(r[0], r[1], r[2], r[3]);
-        } else {
-          float4 R = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (need_res) R = *pr;
-          const float4 Q = *pq;
-          R.x = fmaf(p.a, R.x, p.dt * r[0]); R.y = fmaf(p.a, R.y, p.dt * r[1]);
-          R.z = fmaf(p.a, R.z, p.dt * r[2]); R.w = fmaf(p.a, R.w, p.dt * r[3]);
-          *pr = R;
-          *pq = make_float4(fmaf(p.b, R.x, Q.x), fmaf(p.b, R.y, Q.y), fmaf(p.b, R.z, Q.z), fmaf(p.b, R.w, Q.w));
-        }
-      }
-      __syncwarp();
-      if (c0 + col < ncv) {
-        const size_t base = ((size_t)k0 * NF + qd * 32) * NP + n0 + c0 + col;
-#pragma unroll 4
-        for (int rr = sub; rr < rmax; rr += RPI) {
-          const size_t idx = base + (size_t)rr * NP;
-          if (MODE == MODE_RHS) {
-            p.rhs[idx] = bR[rr * PITCH + col];
-          } else {
-            p.res[idx] = bR[rr * PITCH + col];
-            p.q_out[idx] = bQ[rr * PITCH + col];
-          }
-        }
-      }
-      __syncwarp();
-      issue(stg, ab, ac0);
-      advance(ab, ac0);
-    }
-    tc::cp_async_wait<0>();
-    }
   } else if (warp < 12) {
     // =================================================== producers: rows a1 + a3, BF16x3 split, tcgen05.st
     const int pw = warp - 4, qd = pw & 3, half = pw >> 2;
     const int r = qd * 32 + lane;                      // row = (element e, field f)
     const int e = r / NF, f = r - e * NF;
     const uint32_t trow = tm + ((uint32_t)(qd * 32) << 16) + C::ABASE + 4 * half;
-    constexpr bool VEC4 = (NP % 4) == 0;
     int slot = 0;
     uint32_t phase = 0;
     // One k-step of this row -> TMEM.  The completion of the tcgen05.st (wait::st, fence, arrive) of a k-step is
@@ -523,7 +424,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       T3_WAIT(qFull(qs), quse & 1, 1);
       const unsigned char *sl = s_slot + qs * C::SLOT;
       const float *s_geo = reinterpret_cast<const float *>(sl + (TILE ? C::TILE_SLOT : 0));
-      const float *qb = TILE ? reinterpret_cast<const float *>(sl + tile_shift(k0)) : p.q_in + (size_t)k0 * NF * NP;
+      const float *qb = TILE ? reinterpret_cast<const float *>(sl) : p.q_in + (size_t)k0 * NF * PT;
       auto ldq = [&](const float *x) { return TILE ? *x : __ldg(x); };
       float cf[3][3];
       int src[3] = {0, 0, 0}, nsrc = 0;
@@ -539,7 +440,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       float mean[3];
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
-        sp[i] = qb + (e * NF + src[i]) * NP;
+        sp[i] = qb + (e * NF + src[i]) * PT;
         // mean of the four vertex values: D_j 1 = 0, so the shift is exact and removes the cancellation
         mean[i] = (valid && i < nsrc) ? 0.25f * ((ldq(sp[i]) + ldq(sp[i] + N)) + (ldq(sp[i] + C::NFP - 1) + ldq(sp[i] + NP - 1))) : 0.f;
       }
@@ -547,22 +448,17 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         const int m0 = 16 * g + 8 * half;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-          if (valid && i < nsrc && m0 < NP) {
-            if (VEC4) {
+          if (valid && i < nsrc && m0 < NP) {     // float4 reads: rows are 16-byte aligned (pitch PT), pad columns are zero
 #pragma unroll
-              for (int h4 = 0; h4 < 2; ++h4) {
-                if (m0 + 4 * h4 < NP) {
-                  const float4 v = TILE ? *reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4)
-                                        : __ldg(reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4));
-                  u[i][4 * h4 + 0] = v.x - mean[i]; u[i][4 * h4 + 1] = v.y - mean[i];
-                  u[i][4 * h4 + 2] = v.z - mean[i]; u[i][4 * h4 + 3] = v.w - mean[i];
-                } else {
-                  u[i][4 * h4 + 0] = u[i][4 * h4 + 1] = u[i][4 * h4 + 2] = u[i][4 * h4 + 3] = 0.f;
-                }
+            for (int h4 = 0; h4 < 2; ++h4) {
+              if (m0 + 4 * h4 < NP) {
+                const float4 v = TILE ? *reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4)
+                                      : __ldg(reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4));
+                u[i][4 * h4 + 0] = v.x - mean[i]; u[i][4 * h4 + 1] = v.y - mean[i];
+                u[i][4 * h4 + 2] = v.z - mean[i]; u[i][4 * h4 + 3] = v.w - mean[i];
+              } else {
+                u[i][4 * h4 + 0] = u[i][4 * h4 + 1] = u[i][4 * h4 + 2] = u[i][4 * h4 + 3] = 0.f;
               }
-            } else {
-#pragma unroll
-              for (int t = 0; t < 8; ++t) u[i][t] = (m0 + t < NP) ? ldq(sp[i] + m0 + t) - mean[i] : 0.f;
             }
           } else {
 #pragma unroll
@@ -632,8 +528,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       const unsigned char *sl = s_slot + qs * C::SLOT;
       const float *s_geo = reinterpret_cast<const float *>(sl + (TILE ? C::TILE_SLOT : 0));
       const int *s_conn = reinterpret_cast<const int *>(s_geo + EB * NGEO);
-      const float *s_q = reinterpret_cast<const float *>(sl + tile_shift(k0));        // TILE only
-      const float *gq = p.q_in + (size_t)k0 * NF * NP;                                 // the same values in global memory
+      const float *s_q = reinterpret_cast<const float *>(sl);        // TILE only
+      const float *gq = p.q_in + (size_t)k0 * NF * PT;                                 // the same values in global memory
 #pragma unroll 1
       for (int h = 0; h < C::NH; ++h, ++fc) {
         const int fs = fc % NFL, fuse = fc / NFL;
@@ -656,13 +552,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
               const int nn = __ldg(p.nbrnode + (f * 24 + (c4 & 31)) * NFP + (j - f * NFP));
               const unsigned rel = (unsigned)(nb - k0);
               if (TILE && rel < (unsigned)nvalid) {    // neighbour inside the batch: its values are in the tile
-                const float *qp = s_q + (rel * NF) * NP + nn;
+                const float *qp = s_q + (rel * NF) * PT + nn;
 #pragma unroll
-                for (int c = 0; c < NF; ++c) ext[i][c] = qp[c * NP];
+                for (int c = 0; c < NF; ++c) ext[i][c] = qp[c * PT];
               } else {
-                const float *qp = p.q_in + ((size_t)nb * NF) * NP + nn;
+                const float *qp = p.q_in + ((size_t)nb * NF) * PT + nn;
 #pragma unroll
-                for (int c = 0; c < NF; ++c) ext[i][c] = __ldg(qp + c * NP);
+                for (int c = 0; c < NF; ++c) ext[i][c] = __ldg(qp + c * PT);
               }
             }
           }
@@ -680,13 +576,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
           const int nm = __ldg(p.fmask + j);
           float um[NF];
           if (TILE) {
-            const float *qm = s_q + (e * NF) * NP + nm;
+            const float *qm = s_q + (e * NF) * PT + nm;
 #pragma unroll
-            for (int c = 0; c < NF; ++c) um[c] = qm[c * NP];
+            for (int c = 0; c < NF; ++c) um[c] = qm[c * PT];
           } else {
-            const float *qm = gq + (e * NF) * NP + nm;
+            const float *qm = gq + (e * NF) * PT + nm;
 #pragma unroll
-            for (int c = 0; c < NF; ++c) um[c] = __ldg(qm + c * NP);
+            for (int c = 0; c < NF; ++c) um[c] = __ldg(qm + c * PT);
           }
           float F[NF];
           if (MODEL == 0) {
@@ -786,24 +682,19 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       const int qs = it % NQ, quse = it / NQ;
       T3_WAIT(qEmpty(qs), (quse & 1) ^ 1, 0);
       unsigned char *sl = s_slot + qs * C::SLOT;
-      // 16-byte aligned part [s_al, e_al) of the batch's byte range [s, e) of q; the (< 16 byte) tail by hand
-      const size_t s = (size_t)k0 * NF * NP * 4, e = s + (size_t)nvalid * NF * NP * 4;
-      const size_t s_al = s & ~(size_t)15, e_al = e & ~(size_t)15;
-      if (TILE) {
-        for (size_t x = e_al + 4 * lane; x < e; x += 128)
-          *reinterpret_cast<float *>(sl + (x - s_al)) = __ldg(reinterpret_cast<const float *>(reinterpret_cast<const char *>(p.q_in) + x));
-        __syncwarp();
-      }
-      if (lane == 0) {
-        const uint32_t bq = TILE ? (uint32_t)(e_al - s_al) : 0u, bg = (uint32_t)nvalid * NGEO * 4u, bc = (uint32_t)nvalid * 16u;
+      if (tc::elect_one()) {
+        // rows are 16-byte aligned (pitch PT): the batch's fields are one aligned, contiguous run
+        const float *src = p.q_in + (size_t)k0 * NF * PT;
+        const uint32_t bq = (uint32_t)nvalid * NF * PT * 4u, bg = (uint32_t)nvalid * NGEO * 4u, bc = (uint32_t)nvalid * 16u;
         unsigned char *s_geo = sl + (TILE ? C::TILE_SLOT : 0);
-        tc::mbar_expect_tx(qFull(qs), bq + bg + bc);
-        if (TILE) tc::bulk_g2s(tc::smem_u32(sl), reinterpret_cast<const char *>(p.q_in) + s_al, bq, qFull(qs));
+        tc::mbar_expect_tx(qFull(qs), (TILE ? bq : 0u) + bg + bc);
+        if (TILE) tc::bulk_g2s(tc::smem_u32(sl), src, bq, qFull(qs));
         tc::bulk_g2s(tc::smem_u32(s_geo), p.geo + (size_t)k0 * NGEO, bg, qFull(qs));
         tc::bulk_g2s(tc::smem_u32(s_geo + EB * NGEO * 4), P.conn + (size_t)k0 * 4, bc, qFull(qs));
-        if (!TILE) tc::prefetch_l2(reinterpret_cast<const char *>(p.q_in) + s_al, (uint32_t)(e_al - s_al));
-        if (MODE == MODE_STAGE && p.a != 0.f) tc::prefetch_l2(reinterpret_cast<const char *>(p.res) + s_al, (uint32_t)(e_al - s_al));
+        if (!TILE) tc::prefetch_l2(src, bq);
+        if (MODE == MODE_STAGE && p.a != 0.f) tc::prefetch_l2(p.res + (size_t)k0 * NF * PT, bq);
       }
+      __syncwarp();
     }
   }
 
