@@ -107,7 +107,7 @@ struct dg_ctx {
   int epi_cw = 0;                                // tc3: epilogue chunk width (TMA box columns)
   int PT = 0;                                    // tc3: row pitch (floats) of the arrays the kernel works on, Np rounded up to 4
   float *d_qa = nullptr;                         // tc3, PT != Np: padded private copies of the state (d_qa and d_q2 ping-pong)
-  std::map<const void *, std::array<CUtensorMap, 2>> tmaps;   // device array -> descriptors (box heights 32 / Nf EB - 96)
+  std::map<const void *, std::array<CUtensorMap, 3>> tmaps;   // device array -> descriptors (epilogue boxes of height 32 / Nf EB - 96; field chunks)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
   // launch configuration
@@ -280,7 +280,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-const std::array<CUtensorMap, 2> &tensor_maps(dg_ctx *c, const void *ptr) {
+const std::array<CUtensorMap, 3> &tensor_maps(dg_ctx *c, const void *ptr) {
   auto it = c->tmaps.find(ptr);
   if (it != c->tmaps.end()) return it->second;
   static encode_tiled_fn encode = nullptr;
@@ -292,16 +292,16 @@ const std::array<CUtensorMap, 2> &tensor_maps(dg_ctx *c, const void *ptr) {
     encode = (encode_tiled_fn)fn;
   }
   if (c->tmaps.size() > 32) c->tmaps.clear();
-  std::array<CUtensorMap, 2> m;
+  std::array<CUtensorMap, 3> m;
   const int EB = TC3_INFO[c->model][c->N](1);
   const int rlast = c->NF * EB - 96;
-  for (int h = 0; h < 2; ++h) {
+  for (int h = 0; h < 3; ++h) {          // [2]: field chunks of 16 nodes x 128 rows for the producers (no-tile configurations)
     const cuuint64_t dims[2] = {(cuuint64_t)c->PT, (cuuint64_t)c->K * c->NF};
     const cuuint64_t strides[1] = {(cuuint64_t)c->PT * 4};
-    const cuuint32_t box[2] = {(cuuint32_t)c->epi_cw, (cuuint32_t)(h ? rlast : 32)};
+    const cuuint32_t box[2] = {(cuuint32_t)(h == 2 ? 16 : c->epi_cw), (cuuint32_t)(h == 2 ? 128 : (h ? rlast : 32))};
     const cuuint32_t es[2] = {1, 1};
     const CUresult r = encode(&m[h], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(ptr), dims, strides, box, es,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, c->epi_cw == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, (h < 2 && c->epi_cw == 32) ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) throw std::runtime_error("cuda: cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
   }
@@ -327,6 +327,7 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
       try {
         const auto &mi = tensor_maps(c, q_in), &mr = tensor_maps(c, c->d_res), &mo = tensor_maps(c, q_out ? q_out : rhs);
         for (int h = 0; h < 2; ++h) { tp3.tm_in[h] = mi[h]; tp3.tm_res[h] = mr[h]; tp3.tm_out[h] = mo[h]; }
+        tp3.tm_u = mi[2];
       } catch (const std::exception &e) {
         return fail(DG_ERR_CUDA, e.what());
       }

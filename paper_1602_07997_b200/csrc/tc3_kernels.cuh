@@ -40,6 +40,8 @@ constexpr int T3_W_OPS = 12 + T3_FLUXW, T3_W_MMA = T3_W_OPS + 1, T3_W_LOAD = T3_
 constexpr int T3_THREADS = (T3_W_LOAD + 1) * 32;
 constexpr int T3_NB = 4;             // operator ring stages (shared memory)
 constexpr int T3_NFL = 4;            // flux chunk ring stages (shared memory)
+constexpr int T3_NU = 4;             // field chunk ring stages (shared memory; only when the whole tile does not fit)
+constexpr int T3_UCH = 128 * 16 * 4;  // bytes of one field chunk: 128 rows x 16 nodes
 constexpr int T3_ASTRIDE = 24;       // TMEM columns per A stage: 3 pieces x 8 columns (16 bf16)
 constexpr int T3_FLS = 20;           // floats per row of a flux chunk (16 + pad; 80-byte rows: conflict-free float4)
 constexpr int T3_SMEM_LIMIT = 227 * 1024 - 512;
@@ -69,17 +71,19 @@ struct T3 {
   static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
   static constexpr int CW = NC >= 128 ? 16 : 32;               // epilogue chunk width (output nodes)
   static constexpr int SCR = 4 * 4 * 32 * (CW + 4) * 4;        // per epilogue warp: [stage 2][res | q][32][CW + 4] floats
-  static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4 + 8;
+  static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4 + 8 + 2 * T3_NU;
   static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 1024;
   static constexpr int TILE_SLOT = TILE_RAW;
   static constexpr bool TILE = FIXED + TILE_SLOT + META <= T3_SMEM_LIMIT;   // field tile staged in shared memory
   static constexpr int NQ = !TILE ? 2 : (FIXED + 2 * (TILE_SLOT + META) <= T3_SMEM_LIMIT ? 2 : 1);
   static constexpr int SLOT = (TILE ? TILE_SLOT : 0) + META;   // bytes of one tile slot
+  static constexpr int URING = TILE ? 0 : T3_NU * T3_UCH;      // field chunk ring (TMA boxes of 16 nodes x 128 rows)
   // shared-memory carve-up (bytes)
   static constexpr int OFF_B = 0;
   static constexpr int OFF_FLUX = OFF_B + T3_NB * BSTAGE;
   static constexpr int OFF_SCR = OFF_FLUX + T3_NFL * FLUX_SLOT;
-  static constexpr int OFF_SLOT = OFF_SCR + SCR;
+  static constexpr int OFF_U = OFF_SCR + SCR;
+  static constexpr int OFF_SLOT = OFF_U + URING;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
   static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 1024;  // + slack for the 1024-byte alignment (swizzled TMA boxes)
   static constexpr int TPT = (EB * 16 + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
@@ -121,6 +125,7 @@ struct Tc3Params {
   // epilogue TMA descriptors: 2-D views [K Nf rows][PT] of q_in, res and q_out | rhs with
   // boxes of CW nodes x 32 rows ([0]) and CW x (Nf EB - 96) rows ([1], the last row quadrant of an elastic batch)
   CUtensorMap tm_in[2], tm_res[2], tm_out[2];
+  CUtensorMap tm_u;                    // q_in, boxes of 16 nodes x 128 rows, 64 B swizzle: the producers' field chunks (no tile)
 };
 
 namespace tc {
@@ -241,6 +246,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
   unsigned char *sB = sm + C::OFF_B;                               // [NB][3][2][NCH][8] bf16
   float *s_flux = reinterpret_cast<float *>(sm + C::OFF_FLUX);     // [NFL][128][FLS] penalty-term chunks
   float *s_scr = reinterpret_cast<float *>(sm + C::OFF_SCR);       // epilogue staging (see the epilogue)
+  unsigned char *s_u = sm + C::OFF_U;                              // [NU][128 rows][16] field chunks, 64 B swizzle
   unsigned char *s_slot = sm + C::OFF_SLOT;                        // [NQ] { field tile | geo | conn }
   uint64_t *bars = reinterpret_cast<uint64_t *>(sm + C::OFF_BAR);
   uint32_t *s_tmem = reinterpret_cast<uint32_t *>(bars + C::NBAR);
@@ -261,6 +267,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
   auto qFull = [&](int t) { return barX + 8u * (4 + t); };
   auto qEmpty = [&](int t) { return barX + 8u * (6 + t); };
   auto epiFull = [&](int w, int t) { return barX + 8u * (8 + 2 * w + t); };
+  auto uFull = [&](int t) { return barX + 8u * (16 + t); };
+  auto uEmpty = [&](int t) { return barX + 8u * (16 + T3_NU + t); };
 
   if (warp == T3_W_MMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(s_tmem)), "n"(512) : "memory");
@@ -275,6 +283,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       tc::mbar_init(qFull(t), 1); tc::mbar_init(qEmpty(t), 8 + T3_FLUXW);
       for (int w = 0; w < 4; ++w) tc::mbar_init(epiFull(w, t), 1);
     }
+    for (int t = 0; t < T3_NU; ++t) { tc::mbar_init(uFull(t), 1); tc::mbar_init(uEmpty(t), 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   tc::tc_fence_before();
@@ -415,7 +424,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       pend = slot;
       if (++slot == NA) { slot = 0; phase ^= 1; }
     };
-    int it = 0, fc = 0;
+    int it = 0, fc = 0, uc = 0;
     for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
@@ -466,15 +475,43 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
           }
         }
       };
-      float u[3][8];
-      if (!TILE) load_u(0, u);
+      // without a tile the loader streams the fields as chunks of 16 nodes x 128 rows (64 B swizzle) through a ring
+      auto load_u_ring = [&](int g, const unsigned char *ring, float (&u)[3][8]) {
+        const int m0 = 16 * g + 8 * half;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          if (valid && i < nsrc && m0 < NP) {
+            const int rs = e * NF + src[i];
+            const unsigned char *rowp = ring + rs * 64;
+            const int sw = (rs >> 1) & 3;
+#pragma unroll
+            for (int h4 = 0; h4 < 2; ++h4) {
+              if (m0 + 4 * h4 < NP) {
+                const float4 v = *reinterpret_cast<const float4 *>(rowp + (((2 * half + h4) ^ sw) << 4));
+                u[i][4 * h4 + 0] = v.x - mean[i]; u[i][4 * h4 + 1] = v.y - mean[i];
+                u[i][4 * h4 + 2] = v.z - mean[i]; u[i][4 * h4 + 3] = v.w - mean[i];
+              } else {
+                u[i][4 * h4 + 0] = u[i][4 * h4 + 1] = u[i][4 * h4 + 2] = u[i][4 * h4 + 3] = 0.f;
+              }
+            }
+          } else {
+#pragma unroll
+            for (int t = 0; t < 8; ++t) u[i][t] = 0.f;
+          }
+        }
+      };
 #pragma unroll 1
       for (int g = 0; g < C::NG; ++g) {
-        float un[3][8];
+        float u[3][8];
         if (TILE) {
           load_u(g, u);
-        } else if (g + 1 < C::NG) {
-          load_u(g + 1, un);                           // global reads: one chunk ahead of its use
+        } else {
+          const int us = uc % T3_NU, uuse = uc / T3_NU;
+          ++uc;
+          T3_WAIT(uFull(us), uuse & 1, 1);
+          load_u_ring(g, s_u + us * T3_UCH, u);
+          __syncwarp();
+          if (lane == 0) tc::mbar_arrive(uEmpty(us));
         }
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
@@ -482,12 +519,6 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #pragma unroll
           for (int t = 0; t < 8; ++t) a[t] = cf[j][0] * u[0][t] + cf[j][1] * u[1][t] + cf[j][2] * u[2][t];
           emit(a);
-        }
-        if (!TILE) {
-#pragma unroll
-          for (int i = 0; i < 3; ++i)
-#pragma unroll
-            for (int t = 0; t < 8; ++t) u[i][t] = un[i][t];
         }
       }
       __syncwarp();
@@ -675,7 +706,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     }
   } else {
     // =================================================== tile loader: fields, geometric records, connectivity
-    int it = 0;
+    int it = 0, uc = 0;
     for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
@@ -691,10 +722,20 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         if (TILE) tc::bulk_g2s(tc::smem_u32(sl), src, bq, qFull(qs));
         tc::bulk_g2s(tc::smem_u32(s_geo), p.geo + (size_t)k0 * NGEO, bg, qFull(qs));
         tc::bulk_g2s(tc::smem_u32(s_geo + EB * NGEO * 4), P.conn + (size_t)k0 * 4, bc, qFull(qs));
-        if (!TILE) tc::prefetch_l2(src, bq);
         if (MODE == MODE_STAGE && p.a != 0.f) tc::prefetch_l2(p.res + (size_t)k0 * NF * PT, bq);
       }
       __syncwarp();
+      if (!TILE) {
+        for (int g = 0; g < C::NG; ++g, ++uc) {          // the batch's fields, 16 nodes at a time
+          const int us = uc % T3_NU, uuse = uc / T3_NU;
+          T3_WAIT(uEmpty(us), (uuse & 1) ^ 1, 1);
+          if (tc::elect_one()) {
+            tc::mbar_expect_tx(uFull(us), T3_UCH);
+            tc::tma_load_2d(tc::smem_u32(s_u + us * T3_UCH), &P.tm_u, 16 * g, k0 * NF, uFull(us));
+          }
+          __syncwarp();
+        }
+      }
     }
   }
 
