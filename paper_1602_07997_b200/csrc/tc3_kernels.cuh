@@ -38,8 +38,6 @@ namespace dgk {
 constexpr int T3_FLUXW = 8;           // flux warps
 constexpr int T3_W_OPS = 12 + T3_FLUXW, T3_W_MMA = T3_W_OPS + 1, T3_W_LOAD = T3_W_OPS + 2;   // single-warp roles
 constexpr int T3_THREADS = (T3_W_LOAD + 1) * 32;
-constexpr int T3_NB = 4;             // operator ring stages (shared memory)
-constexpr int T3_NFL = 4;            // flux chunk ring stages (shared memory)
 constexpr int T3_NU = 4;             // field chunk ring stages (shared memory; only when the whole tile does not fit)
 constexpr int T3_UCH = 128 * 16 * 4;  // bytes of one field chunk: 128 rows x 16 nodes
 constexpr int T3_ASTRIDE = 24;       // TMEM columns per A stage: 3 pieces x 8 columns (16 bf16)
@@ -58,6 +56,8 @@ struct T3 {
   static constexpr int NC = (NP + 15) / 16 * 16;               // output nodes, padded
   static constexpr int NSPLIT = NC > 176 ? 2 : 1;              // CTAs sharing one batch (output-node halves)
   static constexpr int NCH = NC / NSPLIT;                      // MMA N of one CTA
+  static constexpr int NB = NCH >= 144 ? 3 : 4;                // operator ring stages (shared memory)
+  static constexpr int NFL = NC >= 176 ? 8 : 4;                // flux chunk ring stages: enough to cover the producers' volume phase
   static constexpr int NG = (NP + 15) / 16;                    // node chunks of 16
   static constexpr int NH = (NFACE + 15) / 16;                 // face-node chunks of 16
   static constexpr int NSTEP = 3 * NG + NH;                    // k-steps of 16 per batch
@@ -70,9 +70,10 @@ struct T3 {
   static constexpr int META = EB * NGEO * 4 + EB * 16;         // geometric records + packed connectivity
   static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
   static constexpr int CW = NC >= 128 ? 16 : 32;               // epilogue chunk width (output nodes)
-  static constexpr int SCR = 4 * 4 * 32 * (CW + 4) * 4;        // per epilogue warp: [stage 2][res | q][32][CW + 4] floats
-  static constexpr int NBAR = 2 * NA + 2 * T3_NB + 2 * T3_NFL + 4 + 4 + 8 + 2 * T3_NU;
-  static constexpr int FIXED = T3_NB * BSTAGE + T3_NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 1024;
+  static constexpr int NES = CW == 16 ? 3 : 2;                 // epilogue staging stages
+  static constexpr int SCR = 4 * NES * 2 * 32 * CW * 4;        // per epilogue warp: [stage][res | q][32 rows][CW] floats (swizzled)
+  static constexpr int NBAR = 2 * NA + 2 * NB + 2 * NFL + 4 + 4 + 12 + 2 * T3_NU;
+  static constexpr int FIXED = NB * BSTAGE + NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 1024;
   static constexpr int TILE_SLOT = TILE_RAW;
   static constexpr bool TILE = FIXED + TILE_SLOT + META <= T3_SMEM_LIMIT;   // field tile staged in shared memory
   static constexpr int NQ = !TILE ? 2 : (FIXED + 2 * (TILE_SLOT + META) <= T3_SMEM_LIMIT ? 2 : 1);
@@ -80,8 +81,8 @@ struct T3 {
   static constexpr int URING = TILE ? 0 : T3_NU * T3_UCH;      // field chunk ring (TMA boxes of 16 nodes x 128 rows)
   // shared-memory carve-up (bytes)
   static constexpr int OFF_B = 0;
-  static constexpr int OFF_FLUX = OFF_B + T3_NB * BSTAGE;
-  static constexpr int OFF_SCR = OFF_FLUX + T3_NFL * FLUX_SLOT;
+  static constexpr int OFF_FLUX = OFF_B + NB * BSTAGE;
+  static constexpr int OFF_SCR = OFF_FLUX + NFL * FLUX_SLOT;
   static constexpr int OFF_U = OFF_SCR + SCR;
   static constexpr int OFF_SLOT = OFF_U + URING;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
@@ -168,7 +169,8 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, int x, int 
                : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+template <int NPEND>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(NPEND) : "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void *src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
@@ -237,7 +239,7 @@ template <int MODEL, int N, int MODE>
 __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_constant__ Tc3Params P) {
   using C = T3<MODEL, N>;
   constexpr int NP = C::NP, PT = C::PT, NFP = C::NFP, NFACE = C::NFACE, NF = C::NF, NGEO = C::NGEO, EB = C::EB, NCH = C::NCH;
-  constexpr int NA = C::NA, NB = T3_NB, NFL = T3_NFL, NQ = C::NQ;
+  constexpr int NA = C::NA, NB = C::NB, NFL = C::NFL, NQ = C::NQ;
   constexpr bool TILE = C::TILE;
   const StageParams &p = P.s;
 
@@ -266,9 +268,9 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
   auto accEmpty = [&](int t) { return barX + 8u * (2 + t); };
   auto qFull = [&](int t) { return barX + 8u * (4 + t); };
   auto qEmpty = [&](int t) { return barX + 8u * (6 + t); };
-  auto epiFull = [&](int w, int t) { return barX + 8u * (8 + 2 * w + t); };
-  auto uFull = [&](int t) { return barX + 8u * (16 + t); };
-  auto uEmpty = [&](int t) { return barX + 8u * (16 + T3_NU + t); };
+  auto epiFull = [&](int w, int t) { return barX + 8u * (8 + 3 * w + t); };
+  auto uFull = [&](int t) { return barX + 8u * (20 + t); };
+  auto uEmpty = [&](int t) { return barX + 8u * (20 + T3_NU + t); };
 
   if (warp == T3_W_MMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc::smem_u32(s_tmem)), "n"(512) : "memory");
@@ -281,8 +283,9 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     for (int t = 0; t < 2; ++t) {
       tc::mbar_init(accFull(t), 1); tc::mbar_init(accEmpty(t), 4);
       tc::mbar_init(qFull(t), 1); tc::mbar_init(qEmpty(t), 8 + T3_FLUXW);
-      for (int w = 0; w < 4; ++w) tc::mbar_init(epiFull(w, t), 1);
     }
+    for (int w = 0; w < 4; ++w)
+      for (int t = 0; t < 3; ++t) tc::mbar_init(epiFull(w, t), 1);
     for (int t = 0; t < T3_NU; ++t) { tc::mbar_init(uFull(t), 1); tc::mbar_init(uEmpty(t), 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -306,7 +309,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     const int qd = warp;
     const int hmap = (qd == 3 && RLAST != 32) ? 1 : 0; // which box height
     const uint32_t boxbytes = (uint32_t)((hmap ? RLAST : 32) * CW * 4);
-    unsigned char *bufs = reinterpret_cast<unsigned char *>(s_scr) + warp * (4 * BUFB);   // [stage 2][res | q]
+    constexpr int NES = C::NES;
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(s_scr) + warp * (NES * 2 * BUFB);   // [stage][res | q]
     const int n0 = hid * NCH;
     const int ncv = min(NCH, NP - n0);
     const bool need_res = MODE == MODE_STAGE && p.a != 0.f;
@@ -329,9 +333,9 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     advance(ab, ac0);
     issue(1, ab, ac0);
     advance(ab, ac0);
-    int it = -1, stg = 0, set = 0;
-    uint32_t par[2] = {0, 0};
-    for (int b = worker, c0 = 0; b < P.nbatch; advance(b, c0), stg ^= 1) {
+    int it = -1, stg = 0, astg = 2 % NES, set = 0;     // stage of the current chunk / of the chunk two ahead
+    uint32_t par = 0;                                  // phase bit per stage
+    for (int b = worker, c0 = 0; b < P.nbatch; advance(b, c0), stg = (stg + 1 == NES ? 0 : stg + 1)) {
       if (c0 == 0) {
         ++it;
         set = C::NSETS == 2 ? (it & 1) : 0;
@@ -347,8 +351,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         if (lane == 0) tc::mbar_arrive(accEmpty(set));
       }
       if (MODE == MODE_STAGE) {
-        T3_WAIT(epiFull(warp, stg), par[stg], 1);      // this chunk's boxes have landed
-        par[stg] ^= 1;
+        T3_WAIT(epiFull(warp, stg), (par >> stg) & 1, 1);   // this chunk's boxes have landed
+        par ^= 1u << stg;
       }
       unsigned char *bR = bufs + (stg * 2) * BUFB, *bQ = bR + BUFB;
       // swizzle: 16-byte chunk j4 of row `lane` sits at chunk j4 ^ f(lane) (128B: lane & 7, 64B: (lane >> 1) & 3)
@@ -383,10 +387,11 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
           tc::tma_store_2d(&P.tm_out[hmap], n0 + c0, row0, tc::smem_u32(bQ));
         }
         tc::bulk_commit();
-        tc::bulk_wait_read0();           // the stores have read the staging buffers: the stage can be refilled
+        tc::bulk_wait_read<NES - 2>();   // the stores of the stage refilled next have read their staging buffers
       }
       __syncwarp();
-      issue(stg, ab, ac0);
+      issue(astg, ab, ac0);
+      astg = astg + 1 == NES ? 0 : astg + 1;
       advance(ab, ac0);
     }
     if (leader) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
