@@ -229,9 +229,9 @@ void build_tc3_image(const dgh::RefElem &ref, int NCH, int nsplit, int nstep, st
 
 void choose_variant(dg_ctx *c, const dg_options *o) {
   int want = o ? o->variant : 0;
-  // auto: the tensor-core kernel wins everywhere in the config-4 sweep except elastic N = 1
-  // (Np = 4: three of four k-steps are padding), where the fused SIMT kernel is faster
-  if (want == 0) want = ((c->N >= 2 || c->model == DG_ACOUSTIC) && c->K < (1 << 26)) ? 4 : 1;
+  // auto (config-4 sweep): the tensor-core kernel from N = 3 up and for elastic N = 2; at N = 1 (Np = 4:
+  // three of four k-steps are padding) and acoustic N = 2 the fused SIMT kernel with one element per thread is faster
+  if (want == 0) want = ((c->N >= 3 || (c->N == 2 && c->model == DG_ELASTIC)) && c->K < (1 << 26)) ? 4 : 1;
   if (want != 1 && want != 4) throw std::invalid_argument("unknown variant (0 auto, 1 fused FP32 SIMT, 4 pipelined tensor core BF16x3)");
   if (want == 4) {
     if (c->K >= (1 << 26)) throw std::invalid_argument("pipelined tensor-core variant packs the neighbour in 26 bits: K < 2^26");
@@ -253,8 +253,12 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     return;
   }
   const int Np = c->Np;
-  int E = (o && o->elems_per_thread > 0) ? o->elems_per_thread : (c->model == DG_ACOUSTIC ? 4 : 2);
-  int G = (o && o->groups_per_cta > 0) ? o->groups_per_cta : std::max(1, std::min(32, (224 + Np / 2) / Np));
+  // register blocking E and node groups G per CTA: at N <= 2 small batches win (more CTAs per SM hide the gather latency;
+  // measured on the config-4 meshes: N = 1 E1 G16 1.34 ms vs E4 G32 2.70 ms per stage)
+  const int E_auto = c->N == 1 ? 1 : (c->N == 2 ? (c->model == DG_ACOUSTIC ? 2 : 1) : (c->model == DG_ACOUSTIC ? 4 : 2));
+  const int G_auto = c->N == 1 ? 16 : (c->N == 2 ? 8 : std::max(1, std::min(32, (224 + Np / 2) / Np)));
+  int E = (o && o->elems_per_thread > 0) ? o->elems_per_thread : E_auto;
+  int G = (o && o->groups_per_cta > 0) ? o->groups_per_cta : G_auto;
   if (!(o && o->groups_per_cta > 0)) {
     // keep the batch under ~64 KB of shared memory so several CTAs fit on an SM
     while (G > 1 && SMEM[c->model][c->N](G * E) > 64 * 1024) --G;
