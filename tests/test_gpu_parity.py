@@ -198,3 +198,50 @@ def test_ab3_matches_paper_eq4(dg):
     for _ in range(4):
         timestep.ab3_step(q, hist, dt, case.oracle_rhs)
     assert rel_l2(d_q.cpu().numpy(), q) <= 1e-5
+
+
+def test_padded_private_layout_paths(dg):
+    """Degrees with Np % 4 != 0 (N = 2, 4, 8, 10): the tensor-core kernel works on a private copy of the state with
+    16-byte aligned rows; dg_rhs, dg_run and dg_ab3_step convert on entry / exit.  Elastic N = 4 (Np = 35)."""
+    from oracle import timestep
+    case = Case(dg, _sweep_case(W.ELASTIC, 4), variant=4)
+    assert "pitch=36" in case.ctx.variant_name
+    q32 = case.initial_fields32()
+    dt = case.dt32()
+    got = case.gpu_run(torch, q32, dt, 3)
+    assert case.ctx.last_launch_count == 5 * 3 + 2                  # two layout conversions around the 15 stage kernels
+    assert rel_l2(got, case.oracle_run(q32.astype(np.float64), dt, 3)) <= RUN_TOL
+    # dg_rhs leaves q untouched and fills every entry of rhs (no pad column leaks into the caller's arrays)
+    d_q = torch.from_numpy(q32).cuda()
+    d_r = torch.full_like(d_q, float("nan"))
+    case.ctx.rhs(d_q.data_ptr(), d_r.data_ptr())
+    torch.cuda.synchronize()
+    assert case.ctx.last_launch_count == 3
+    assert np.array_equal(d_q.cpu().numpy(), q32) and np.isfinite(d_r.cpu().numpy()).all()
+    # the paper's AB3 step through the same conversion
+    dta = case.dt32(0.2)
+    case.ctx.ab3_reset()
+    for _ in range(3):
+        case.ctx.ab3_step(d_q.data_ptr(), dta)
+    torch.cuda.synchronize()
+    q = q32.astype(np.float64)
+    hist = [np.zeros_like(q), np.zeros_like(q)]
+    for _ in range(3):
+        timestep.ab3_step(q, hist, dta, case.oracle_rhs)
+    assert rel_l2(d_q.cpu().numpy(), q) <= 1e-5
+
+
+def test_variant_selection_and_errors(dg):
+    """auto picks the SIMT kernel at N = 1 and acoustic N = 2, the tensor-core kernel elsewhere; unknown variants and
+    misaligned device buffers are rejected."""
+    names = {(m, N): Case(dg, _sweep_case(m, N, n=1)).ctx.variant_name for m in (W.ACOUSTIC, W.ELASTIC) for N in (1, 2, 3)}
+    assert names[(W.ACOUSTIC, 1)].startswith("simt_fused") and names[(W.ELASTIC, 1)].startswith("simt_fused")
+    assert names[(W.ACOUSTIC, 2)].startswith("simt_fused") and names[(W.ELASTIC, 2)].startswith("tc_pipe")
+    assert names[(W.ACOUSTIC, 3)].startswith("tc_pipe") and names[(W.ELASTIC, 3)].startswith("tc_pipe")
+    with pytest.raises(dg.DGError):
+        Case(dg, _sweep_case(W.ACOUSTIC, 3, n=1), variant=2)
+    case = Case(dg, _sweep_case(W.ACOUSTIC, 3, n=1), variant=4)
+    buf = torch.zeros(int(np.prod(case.ctx.shape)) + 1, dtype=torch.float32, device="cuda")
+    out = torch.zeros_like(buf)
+    with pytest.raises(dg.DGError):                                  # q not 16-byte aligned
+        case.ctx.rhs(buf.data_ptr() + 4, out.data_ptr())
