@@ -104,7 +104,7 @@ class Context:
 
     # -- lifetime
     def close(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and _lib is not None:      # _lib is None while the interpreter shuts down
             _lib.dg_destroy(self._h)
             self._h = None
 
