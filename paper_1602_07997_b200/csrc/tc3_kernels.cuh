@@ -41,7 +41,6 @@ constexpr int T3_THREADS = (T3_W_LOAD + 1) * 32;
 constexpr int T3_NU = 4;             // field chunk ring stages (shared memory; only when the whole tile does not fit)
 constexpr int T3_UCH = 128 * 16 * 4;  // bytes of one field chunk: 128 rows x 16 nodes
 constexpr int T3_ASTRIDE = 24;       // TMEM columns per A stage: 3 pieces x 8 columns (16 bf16)
-constexpr int T3_FLS = 20;           // floats per row of a flux chunk (16 + pad; 80-byte rows: conflict-free float4)
 constexpr int T3_SMEM_LIMIT = 227 * 1024 - 512;
 
 template <int MODEL, int N>
@@ -57,9 +56,14 @@ struct T3 {
   static constexpr int NSPLIT = NC > 176 ? 2 : 1;              // CTAs sharing one batch (output-node halves)
   static constexpr int NCH = NC / NSPLIT;                      // MMA N of one CTA
   static constexpr int NB = NCH >= 144 ? 3 : 4;                // operator ring stages (shared memory)
-  static constexpr int NFL = NC >= 176 ? 8 : 4;                // flux chunk ring stages: enough to cover the producers' volume phase
+  // flux chunks: 32 face nodes (two k-steps; four tasks in flight per flux thread) from N = 5 up, 16 below, where a
+  // batch has only two to four k-steps of face nodes (measured: N = 3 is 14 % slower with 32, N = 10 9 % faster)
+  static constexpr int FCH = N >= 5 ? 32 : 16;
+  static constexpr int FLS = FCH + 4;                          // floats per row of a chunk (80 / 144-byte rows: conflict-free float4)
+  static constexpr int NFL = FCH == 16 ? 4 : (NC >= 176 ? 4 : 3);                // flux chunk ring stages: enough to cover the producers' volume phase
   static constexpr int NG = (NP + 15) / 16;                    // node chunks of 16
-  static constexpr int NH = (NFACE + 15) / 16;                 // face-node chunks of 16
+  static constexpr int NH = (NFACE + 15) / 16;                 // face-node k-steps of 16
+  static constexpr int NHC = (NFACE + FCH - 1) / FCH;          // flux chunks
   static constexpr int NSTEP = 3 * NG + NH;                    // k-steps of 16 per batch
   static constexpr int NSETS = (4 * NCH + 3 * T3_ASTRIDE <= 512) ? 2 : 1;   // accumulator sets
   static constexpr int ABASE = NSETS * 2 * NCH;                // first TMEM column of the A ring
@@ -68,7 +72,7 @@ struct T3 {
   static constexpr int BSTAGE = 96 * NCH;                      // bytes: [3 pieces][2 kc][NCH][8] bf16
   static constexpr int TILE_RAW = EB * NF * PT * 4;            // bytes of the batch's fields (multiple of 16)
   static constexpr int META = EB * NGEO * 4 + EB * 16;         // geometric records + packed connectivity
-  static constexpr int FLUX_SLOT = 128 * T3_FLS * 4;
+  static constexpr int FLUX_SLOT = 128 * FLS * 4;
   static constexpr int CW = NC >= 128 ? 16 : 32;               // epilogue chunk width (output nodes)
   static constexpr int NES = CW == 16 ? 3 : 2;                 // epilogue staging stages
   static constexpr int SCR = 4 * NES * 2 * 32 * CW * 4;        // per epilogue warp: [stage][res | q][32 rows][CW] floats (swizzled)
@@ -87,7 +91,7 @@ struct T3 {
   static constexpr int OFF_SLOT = OFF_U + URING;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
   static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 1024;  // + slack for the 1024-byte alignment (swizzled TMA boxes)
-  static constexpr int TPT = (EB * 16 + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
+  static constexpr int TPT = (EB * FCH + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
   static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
   static_assert(NA >= 3, "A ring too small");
   static_assert(SMEM <= 227 * 1024, "shared memory");
@@ -343,8 +347,16 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         tc::tc_fence_after();
       }
       const uint32_t t0 = tm + ((uint32_t)(qd * 32) << 16) + set * 2 * NCH + c0;
-      uint32_t vm[CW], vs[CW];
-      T3_TIMED(2, tc::tmem_ld<CW>(t0, vm); tc::tmem_ld<CW>(t0 + NCH, vs));
+      float acc[CW];                     // main + small accumulator, summed 16 columns at a time (register pressure)
+      {
+#pragma unroll
+        for (int h = 0; h < CW / 16; ++h) {
+          uint32_t vm[16], vs[16];
+          T3_TIMED(2, tc::tmem_ld<16>(t0 + 16 * h, vm); tc::tmem_ld<16>(t0 + NCH + 16 * h, vs));
+#pragma unroll
+          for (int j = 0; j < 16; ++j) acc[16 * h + j] = __uint_as_float(vm[j]) + __uint_as_float(vs[j]);
+        }
+      }
       if (c0 + CW >= ncv) {              // accumulators drained: the MMA warp may start the next batch on this set
         tc::tc_fence_before();
         __syncwarp();
@@ -363,7 +375,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         float4 *pr = reinterpret_cast<float4 *>(bR + off), *pq = reinterpret_cast<float4 *>(bQ + off);
         float r[4];
 #pragma unroll
-        for (int t = 0; t < 4; ++t) r[t] = __uint_as_float(vm[4 * j4 + t]) + __uint_as_float(vs[4 * j4 + t]);
+        for (int t = 0; t < 4; ++t) r[t] = acc[4 * j4 + t];
         if (MODE == MODE_RHS) {
           *pr = make_float4(r[0], r[1], r[2], r[3]);
         } else {
@@ -529,11 +541,12 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       __syncwarp();
       if (lane == 0) tc::mbar_arrive(qEmpty(qs));      // this warp no longer reads the tile slot
 #pragma unroll 1
-      for (int h = 0; h < C::NH; ++h, ++fc) {
+      for (int h = 0; h < C::NH; ++h) {
         const int fs = fc % NFL, fuse = fc / NFL;
-        T3_WAIT(flFull(fs), fuse & 1, 2);
+        constexpr int KPC = C::FCH / 16;                              // k-steps per flux chunk
+        if (h % KPC == 0) T3_WAIT(flFull(fs), fuse & 1, 2);
         const int j0 = 16 * h + 8 * half;
-        const float *fl = s_flux + fs * (128 * T3_FLS) + r * T3_FLS + 8 * half;
+        const float *fl = s_flux + fs * (128 * C::FLS) + r * C::FLS + 16 * (h % KPC) + 8 * half;
         float a[8];
         if (valid) {
           const float4 v0 = *reinterpret_cast<const float4 *>(fl);
@@ -545,8 +558,11 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #pragma unroll
           for (int t = 0; t < 8; ++t) a[t] = 0.f;
         }
-        __syncwarp();
-        if (lane == 0) tc::mbar_arrive(flEmpty(fs));
+        if (h % KPC == KPC - 1 || h == C::NH - 1) {                   // done with the chunk
+          __syncwarp();
+          if (lane == 0) tc::mbar_arrive(flEmpty(fs));
+          ++fc;
+        }
         emit(a);
       }
       finish();                                        // the batch's last k-step must not wait for the next batch
@@ -567,7 +583,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       const float *s_q = reinterpret_cast<const float *>(sl);        // TILE only
       const float *gq = p.q_in + (size_t)k0 * NF * PT;                                 // the same values in global memory
 #pragma unroll 1
-      for (int h = 0; h < C::NH; ++h, ++fc) {
+      for (int h = 0; h < C::NHC; ++h, ++fc) {
         const int fs = fc % NFL, fuse = fc / NFL;
         // ---- gather the exterior traces of this thread's tasks (all loads in flight before the first use)
         float ext[TPT][NF];
@@ -575,7 +591,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #pragma unroll
         for (int i = 0; i < TPT; ++i) {
           const int t = ft + T3_FLUXW * 32 * i;
-          const int e = t >> 4, j = 16 * h + (t & 15);
+          const int e = t / C::FCH, j = C::FCH * h + (t % C::FCH);
           cn[i] = (int)0x80000000;
 #pragma unroll
           for (int c = 0; c < NF; ++c) ext[i][c] = 0.f;
@@ -600,13 +616,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
           }
         }
         T3_WAIT(flEmpty(fs), (fuse & 1) ^ 1, 1);    // producers have consumed the chunk that used this slot
-        float *fl = s_flux + fs * (128 * T3_FLS);
+        float *fl = s_flux + fs * (128 * C::FLS);
         // ---- penalty terms
 #pragma unroll
         for (int i = 0; i < TPT; ++i) {
           if (cn[i] == (int)0x80000000) continue;
           const int t = ft + T3_FLUXW * 32 * i;
-          const int e = t >> 4, jj = t & 15, j = 16 * h + jj;
+          const int e = t / C::FCH, jj = t % C::FCH, j = C::FCH * h + jj;
           const int f = j / NFP;
           const float *g = s_geo + e * NGEO;
           const int nm = __ldg(p.fmask + j);
@@ -650,7 +666,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
             elastic_penalty(g, fg, dv, dT, F);
           }
 #pragma unroll
-          for (int c = 0; c < NF; ++c) fl[(e * NF + c) * T3_FLS + jj] = F[c];
+          for (int c = 0; c < NF; ++c) fl[(e * NF + c) * C::FLS + jj] = F[c];
         }
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(flFull(fs));
