@@ -180,6 +180,21 @@ def run_reference(a):
     return 0
 
 
+def max_over_ranks(values_ms, device, world):
+    """Device-timed durations of one replica each -> the slowest rank's (every rank gets the same numbers)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values_ms), device=device, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def whole_job_value(world, nodes_per_replica, stages, ms):
+    """node-updates/s per RK stage summed over `world` independent replicas (weak scaling), timed by the slowest one."""
+    return world * nodes_per_replica * stages / (ms * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------------
 def run_ours(a):
     import torch
@@ -249,14 +264,11 @@ def run_ours(a):
     barrier()
     ms_e2e = e0.elapsed_time(e1)
 
-    t = torch.tensor([ms, ms_e2e], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(t[0]), float(t[1])
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], "cuda", world)
 
     nodes = w.K * w.Np
     stages = 5 * a.steps
-    value = world * nodes * stages / (ms * 1e-3)
+    value = whole_job_value(world, nodes, stages, ms)
     flops = flops_per_element(w.model, w.N) * w.K
     byts = bytes_per_element(w.model, w.N) * w.K
     hbm_peak, bf16_peak, which = measured_peaks()
