@@ -69,7 +69,9 @@ typedef struct {              /* HOST, per element, fp64 (piecewise-constant med
 typedef struct {
   int device;                 /* CUDA device ordinal; -1 = host-only context (setup introspection,
                                  no device entry point works: they return DG_ERR_CUDA)           */
-  int variant;                /* 0 = auto (1 for N = 1 and acoustic N = 2, else 4); 1 = fused FP32 SIMT stage kernel;
+  int variant;                /* 0 = auto (1 for N = 1 and acoustic N = 2, else 4); 1 = FP32 SIMT stage kernels (element per
+                                 thread for acoustic N <= 2 / elastic N = 1, fused node per thread otherwise or when
+                                 elems_per_thread / groups_per_cta is given);
                                  4 = pipelined warp-specialised tensor-core kernel (tcgen05, BF16x3 split, TMEM
                                  accumulators), every degree; needs 16-byte aligned q / rhs and K < 2^26.
                                  Any other value: DG_ERR_ARG                                           */

@@ -23,6 +23,8 @@
   extern "C" const void *dgk_get_stage_kernel_##m##_##n(int, int); \
   extern "C" size_t dgk_stage_smem_bytes_##m##_##n(int);           \
   extern "C" const void *dgk_get_tc3_kernel_##m##_##n(int);       \
+  extern "C" const void *dgk_get_epk_kernel_##m##_##n(int);       \
+  extern "C" int dgk_epk_upload_##m##_##n(const float *, const float *, const unsigned short *, const int *); \
   extern "C" int dgk_tc3_info_##m##_##n(int);
 #define DG_DECL_ALL(m) \
   DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
@@ -46,6 +48,9 @@ typedef int (*info_getter)(int);
    fn##m##_10}
 const kernel_getter KERNELS[2][11] = {DG_ROW(0, dgk_get_stage_kernel_), DG_ROW(1, dgk_get_stage_kernel_)};
 const smem_getter SMEM[2][11] = {DG_ROW(0, dgk_stage_smem_bytes_), DG_ROW(1, dgk_stage_smem_bytes_)};
+typedef int (*epk_upload_fn)(const float *, const float *, const unsigned short *, const int *);
+const tc_getter EPK_KERNELS[2][11] = {DG_ROW(0, dgk_get_epk_kernel_), DG_ROW(1, dgk_get_epk_kernel_)};
+const epk_upload_fn EPK_UPLOAD[2][11] = {DG_ROW(0, dgk_epk_upload_), DG_ROW(1, dgk_epk_upload_)};
 const tc_getter TC3_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc3_kernel_), DG_ROW(1, dgk_get_tc3_kernel_)};
 const info_getter TC3_INFO[2][11] = {DG_ROW(0, dgk_tc3_info_), DG_ROW(1, dgk_tc3_info_)};
 
@@ -103,6 +108,7 @@ struct dg_ctx {
   unsigned short *d_fmask = nullptr, *d_nbrnode = nullptr;
   uint16_t *d_Bimg = nullptr;                    // tensor-core variant: bf16x3 operator panel image
   bool tc3 = false;                              // pipelined BF16x3 tensor-core variant (tc3_kernels.cuh)
+  bool epk = false;                              // element-per-thread kernel (epk_kernels.cuh): acoustic N <= 2, elastic N = 1
   int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
   int epi_cw = 0;                                // tc3: epilogue chunk width (TMA box columns)
   int PT = 0;                                    // tc3: row pitch (floats) of the arrays the kernel works on, Np rounded up to 4
@@ -253,6 +259,19 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     return;
   }
   const int Np = c->Np;
+  // lowest degrees: one element per thread, everything in registers -- unless a launch shape of the generic kernel is asked for
+  if (EPK_KERNELS[c->model][c->N](dgk::MODE_STAGE) && !(o && (o->elems_per_thread > 0 || o->groups_per_cta > 0))) {
+    c->epk = true;
+    c->k_rhs = EPK_KERNELS[c->model][c->N](dgk::MODE_RHS);
+    c->k_stage = EPK_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    c->NT = 128;
+    c->smem = 0;
+    c->grid = (int)((c->K + 127) / 128);
+    char buf[128];
+    snprintf(buf, sizeof buf, "simt_elem_per_thread<%s,N=%d,threads=128,operators in constant memory>", c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N);
+    c->variant = buf;
+    return;
+  }
   // register blocking E and node groups G per CTA: at N <= 2 small batches win (more CTAs per SM hide the gather latency;
   // measured on the config-4 meshes: N = 1 E1 G16 1.34 ms vs E4 G32 2.70 ms per stage)
   const int E_auto = c->N == 1 ? 1 : (c->N == 2 ? (c->model == DG_ACOUSTIC ? 2 : 1) : (c->model == DG_ACOUSTIC ? 4 : 2));
@@ -321,6 +340,8 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
   dgk::Tc3Params tp3;
   void *args[] = {&p};
+  if (c->epk && (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15))
+    return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
   if (c->tc3) {
     if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
     tp3.s = p;
@@ -418,6 +439,17 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
       c->d_fcode = upload(c->mesh.fcode);
       c->d_fmask = upload(fmask);
       c->d_nbrnode = upload(nbrnode);
+      if (c->epk) {
+        std::vector<float> Dm((size_t)3 * Np * Np), Lm((size_t)Np * 4 * Nfp);
+        const std::vector<double> *Ds3[3] = {&c->ref.Dr, &c->ref.Ds, &c->ref.Dt};
+        for (int d = 0; d < 3; ++d)
+          for (size_t i = 0; i < (size_t)Np * Np; ++i) Dm[(size_t)d * Np * Np + i] = (float)(*Ds3[d])[i];
+        for (size_t i = 0; i < Lm.size(); ++i) Lm[i] = (float)c->ref.LIFT[i];
+        std::vector<int> fm(c->ref.fmask.begin(), c->ref.fmask.end());
+        const int rc = EPK_UPLOAD[c->model][c->N](Dm.data(), Lm.data(), nbrnode.data(), fm.data());
+        if (rc == -1) throw std::runtime_error("element-per-thread kernel: face masks differ from the compile-time table");
+        if (rc != 0) throw std::runtime_error(std::string("cuda: ") + cudaGetErrorString((cudaError_t)rc) + " uploading the operators to constant memory");
+      }
       if (c->tc3) {
         const info_getter info = TC3_INFO[c->model][c->N];
         const int nsplit = info(4);

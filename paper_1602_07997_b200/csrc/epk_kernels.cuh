@@ -1,0 +1,245 @@
+// Element-per-thread stage kernel of libdg for the lowest degrees (acoustic N = 1, 2; elastic N = 1).
+//
+// At Np = 4 .. 10 an element's fields fit in one thread's registers (16 .. 40 values), so every row of the hot path
+// (a1-a7) runs without shared memory: the fields and the residual move as 16-byte vectors, the
+// reference operators D_r, D_s, D_t and LIFT sit in constant memory and enter the FFMAs as constant-bank operands (all
+// loops are fully unrolled, every register index is a compile-time constant), and the only irregular access is the gather
+// of the exterior traces through the compressed connectivity.  The generic fused SIMT kernel (kernels.cuh) is bound by
+// its shared-memory operand traffic at these degrees (L1/LSU pipe 98 % busy at N = 1).
+//
+// Prior art: the one-element-per-thread kernels of PAPER.md:173 (K1-K3, element-fastest layout, operators prefetched to
+// shared memory); here the node-fastest ABI layout is kept (an element is one contiguous run), the three kernels are
+// fused with the LSRK update, and the operators need no staging.  The arithmetic (vertex-mean shift, pre-/post-
+// combination order, penalty terms) is the one of kernels.cuh.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "flux.cuh"
+#include "kernels.cuh"
+
+namespace dgk {
+
+constexpr int EPK_MAXNP = 10, EPK_MAXNFP = 6, EPK_MAXNFACE = 24;     // N <= 2
+static __constant__ float c_epk_D[3 * EPK_MAXNP * EPK_MAXNP];          // D_j[n][m] at (j Np + n) Np + m
+static __constant__ float c_epk_L[EPK_MAXNP * EPK_MAXNFACE];           // LIFT[n][j] at n 4Nfp + j
+static __constant__ unsigned short c_epk_nbrnode[4 * 24 * EPK_MAXNFP]; // neighbour's volume node at (f 24 + code) Nfp + i
+
+// face masks in the library's order (host_setup.cpp: nodes in lattice order, t slowest, r fastest; a face lists its
+// nodes by increasing number) as compile-time constants, so that interior traces are register reads
+template <int N>
+struct EpkFmask {
+  static constexpr int NFP = (N + 1) * (N + 2) / 2;
+  int v[4 * NFP];
+  constexpr EpkFmask() : v{} {
+    int cnt[4] = {0, 0, 0, 0};
+    int n = 0;
+    for (int k = 0; k <= N; ++k)
+      for (int j = 0; j <= N - k; ++j)
+        for (int i = 0; i <= N - k - j; ++i, ++n) {
+          if (k == 0) v[0 * NFP + cnt[0]++] = n;             // t = -1
+          if (j == 0) v[1 * NFP + cnt[1]++] = n;             // s = -1
+          if (i + j + k == N) v[2 * NFP + cnt[2]++] = n;     // r + s + t = -1
+          if (i == 0) v[3 * NFP + cnt[3]++] = n;             // r = -1
+        }
+  }
+};
+
+template <int MODEL, int N, int MODE>
+__global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
+  using D = Deg<N>;
+  constexpr int NP = D::NP, NFP = D::NFP, NFACE = D::NFACE;
+  constexpr int NF = MODEL == 0 ? 4 : 9, NGEO = MODEL == 0 ? GEO_AC : GEO_EL;
+  constexpr int NV = NF * NP;                                          // values per element
+  static_assert(NV % 4 == 0, "an element's fields are moved as 16-byte vectors");
+  constexpr EpkFmask<N> FM{};
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= p.K) return;
+
+  // ---- per-element constants and fields
+  const float *g = p.geo + (size_t)k * NGEO;
+  float gl[16];                                                        // G[9], material constants
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float4 v = __ldg(reinterpret_cast<const float4 *>(g) + i);
+    gl[4 * i] = v.x; gl[4 * i + 1] = v.y; gl[4 * i + 2] = v.z; gl[4 * i + 3] = v.w;
+  }
+  float q[NV], r[NV];
+  {
+    const float4 *src = reinterpret_cast<const float4 *>(p.q_in + (size_t)k * NV);
+#pragma unroll
+    for (int i = 0; i < NV / 4; ++i) {
+      const float4 v = __ldg(src + i);
+      q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
+    }
+  }
+
+  // ---- volume term (rows a1-a3).  Inputs of a differentiation are shifted by the mean of the four vertex values
+  // (D_j 1 = 0)
+  float u[NV];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    const float mean = 0.25f * ((q[f * NP] + q[f * NP + N]) + (q[f * NP + NFP - 1] + q[f * NP + NP - 1]));
+#pragma unroll
+    for (int m = 0; m < NP; ++m) u[f * NP + m] = q[f * NP + m] - mean;
+  }
+  if (MODEL == 0) {
+    // eq. (5): w_j = sum_i g_ij v_i
+    float w[3][NP];
+#pragma unroll
+    for (int m = 0; m < NP; ++m) {
+      w[0][m] = gl[0] * u[NP + m] + gl[3] * u[2 * NP + m] + gl[6] * u[3 * NP + m];
+      w[1][m] = gl[1] * u[NP + m] + gl[4] * u[2 * NP + m] + gl[7] * u[3 * NP + m];
+      w[2][m] = gl[2] * u[NP + m] + gl[5] * u[2 * NP + m] + gl[8] * u[3 * NP + m];
+    }
+    const float kap = gl[9], irho = gl[10];
+#pragma unroll
+    for (int n = 0; n < NP; ++n) {
+      float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll
+      for (int m = 0; m < NP; ++m) {
+        const float dr = c_epk_D[(0 * NP + n) * NP + m], ds = c_epk_D[(1 * NP + n) * NP + m], dt = c_epk_D[(2 * NP + n) * NP + m];
+        a0 = fmaf(dr, u[m], a0);
+        a1 = fmaf(ds, u[m], a1);
+        a2 = fmaf(dt, u[m], a2);
+        a3 = fmaf(dr, w[0][m], a3);
+        a3 = fmaf(ds, w[1][m], a3);
+        a3 = fmaf(dt, w[2][m], a3);
+      }
+      // eq. (5)-(6)
+      r[n] = -kap * a3;
+#pragma unroll
+      for (int i = 0; i < 3; ++i) r[(1 + i) * NP + n] = -irho * (gl[3 * i] * a0 + gl[3 * i + 1] * a1 + gl[3 * i + 2] * a2);
+    }
+  } else {
+    // w_{i,n} = sum_m g_mn sigma_im ; fields vx vy vz sxx syy szz sxy sxz syz
+    const float irho = gl[9], lam = gl[10], mu = gl[11];
+    constexpr int SG[3][3] = {{3, 6, 7}, {6, 4, 8}, {7, 8, 5}};
+    float w[3][3][NP];                                                 // w[i][j][m] = sum_c g_cj sigma_ic
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int m = 0; m < NP; ++m) {
+        const float s0 = u[SG[i][0] * NP + m], s1 = u[SG[i][1] * NP + m], s2 = u[SG[i][2] * NP + m];
+        w[i][0][m] = gl[0] * s0 + gl[3] * s1 + gl[6] * s2;
+        w[i][1][m] = gl[1] * s0 + gl[4] * s1 + gl[7] * s2;
+        w[i][2][m] = gl[2] * s0 + gl[5] * s1 + gl[8] * s2;
+      }
+#pragma unroll
+    for (int n = 0; n < NP; ++n) {
+      float acc[12];
+#pragma unroll
+      for (int c = 0; c < 12; ++c) acc[c] = 0.f;
+#pragma unroll
+      for (int m = 0; m < NP; ++m) {
+        const float dr = c_epk_D[(0 * NP + n) * NP + m], ds = c_epk_D[(1 * NP + n) * NP + m], dt = c_epk_D[(2 * NP + n) * NP + m];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          acc[3 * i + 0] = fmaf(dr, u[i * NP + m], acc[3 * i + 0]);
+          acc[3 * i + 1] = fmaf(ds, u[i * NP + m], acc[3 * i + 1]);
+          acc[3 * i + 2] = fmaf(dt, u[i * NP + m], acc[3 * i + 2]);
+          acc[9 + i] = fmaf(dr, w[i][0][m], acc[9 + i]);
+          acc[9 + i] = fmaf(ds, w[i][1][m], acc[9 + i]);
+          acc[9 + i] = fmaf(dt, w[i][2][m], acc[9 + i]);
+        }
+      }
+      float gv[3][3];   // gv[i][j] = d_j v_i = sum_m g_jm (D_m v_i)
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) gv[i][j] = gl[3 * j] * acc[3 * i] + gl[3 * j + 1] * acc[3 * i + 1] + gl[3 * j + 2] * acc[3 * i + 2];
+      const float div = gv[0][0] + gv[1][1] + gv[2][2];
+      r[0 * NP + n] = irho * acc[9];
+      r[1 * NP + n] = irho * acc[10];
+      r[2 * NP + n] = irho * acc[11];
+      r[3 * NP + n] = lam * div + 2.f * mu * gv[0][0];
+      r[4 * NP + n] = lam * div + 2.f * mu * gv[1][1];
+      r[5 * NP + n] = lam * div + 2.f * mu * gv[2][2];
+      r[6 * NP + n] = mu * (gv[0][1] + gv[1][0]);
+      r[7 * NP + n] = mu * (gv[0][2] + gv[2][0]);
+      r[8 * NP + n] = mu * (gv[1][2] + gv[2][1]);
+    }
+  }
+
+  // ---- surface term (rows a4-a6): gather, penalty terms times g^sur, lift
+#pragma unroll
+  for (int f = 0; f < 4; ++f) {
+    constexpr int FO = MODEL == 0 ? 12 : 16, FS = MODEL == 0 ? 5 : 8;
+    float fg[8];
+#pragma unroll
+    for (int i = 0; i < FS; ++i) fg[i] = __ldg(g + FO + FS * f + i);
+    const float nx = fg[0], ny = fg[1], nz = fg[2];
+    const int nb = __ldg(p.nbr + (size_t)k * 4 + f);
+    const int code = (int)__ldg(p.fcode + (size_t)k * 4 + f);
+#pragma unroll
+    for (int i = 0; i < NFP; ++i) {
+      const int j = f * NFP + i;
+      const int nm = FM.v[f * NFP + i];                                // compile-time: q[] stays in registers
+      float um[NF], F[NF];
+#pragma unroll
+      for (int c = 0; c < NF; ++c) um[c] = q[c * NP + nm];
+      if (MODEL == 0) {
+        float dp, dvn;
+        if (nb >= 0) {
+          const int nn = c_epk_nbrnode[(f * 24 + code) * NFP + i];
+          const float *qp = p.q_in + (size_t)nb * NV + nn;
+          dp = __ldg(qp) - um[0];
+          dvn = (__ldg(qp + NP) - um[1]) * nx + (__ldg(qp + 2 * NP) - um[2]) * ny + (__ldg(qp + 3 * NP) - um[3]) * nz;
+        } else {
+          acoustic_boundary_jump(nb, um[0], um[1] * nx + um[2] * ny + um[3] * nz, dp, dvn);
+        }
+        const float4 Pn = acoustic_penalty(gl, fg, dp, dvn);
+        F[0] = Pn.x; F[1] = Pn.y; F[2] = Pn.z; F[3] = Pn.w;
+      } else {
+        float Tmx, Tmy, Tmz;
+        traction(um, nx, ny, nz, Tmx, Tmy, Tmz);
+        float dv[3], dT[3];
+        if (nb >= 0) {
+          const int nn = c_epk_nbrnode[(f * 24 + code) * NFP + i];
+          const float *qp = p.q_in + (size_t)nb * NV + nn;
+          float up[NF];
+#pragma unroll
+          for (int c = 0; c < NF; ++c) up[c] = __ldg(qp + c * NP);
+          float Tpx, Tpy, Tpz;
+          traction(up, nx, ny, nz, Tpx, Tpy, Tpz);
+          dv[0] = up[0] - um[0]; dv[1] = up[1] - um[1]; dv[2] = up[2] - um[2];
+          dT[0] = Tpx - Tmx; dT[1] = Tpy - Tmy; dT[2] = Tpz - Tmz;
+        } else {
+          elastic_boundary_jump(nb, um, Tmx, Tmy, Tmz, nx, ny, nz, dv, dT);
+        }
+        elastic_penalty(gl, fg, dv, dT, F);
+      }
+#pragma unroll
+      for (int n = 0; n < NP; ++n) {
+        const float l = c_epk_L[n * NFACE + j];
+#pragma unroll
+        for (int c = 0; c < NF; ++c) r[c * NP + n] = fmaf(l, F[c], r[c * NP + n]);
+      }
+    }
+  }
+
+  // ---- LSRK update (row a7), 16-byte vectors
+  const size_t base = (size_t)k * NV;
+  if (MODE == MODE_RHS) {
+    float4 *dst = reinterpret_cast<float4 *>(p.rhs + base);
+#pragma unroll
+    for (int i = 0; i < NV / 4; ++i) dst[i] = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+  } else {
+    float4 *pres = reinterpret_cast<float4 *>(p.res + base), *pq = reinterpret_cast<float4 *>(p.q_out + base);
+#pragma unroll
+    for (int i = 0; i < NV / 4; ++i) {
+      float rs[4];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) rs[t] = p.dt * r[4 * i + t];
+      if (p.a != 0.f) {
+        const float4 o = pres[i];
+        rs[0] = fmaf(p.a, o.x, rs[0]); rs[1] = fmaf(p.a, o.y, rs[1]); rs[2] = fmaf(p.a, o.z, rs[2]); rs[3] = fmaf(p.a, o.w, rs[3]);
+      }
+      pres[i] = make_float4(rs[0], rs[1], rs[2], rs[3]);
+      pq[i] = make_float4(fmaf(p.b, rs[0], q[4 * i]), fmaf(p.b, rs[1], q[4 * i + 1]), fmaf(p.b, rs[2], q[4 * i + 2]),
+                          fmaf(p.b, rs[3], q[4 * i + 3]));
+    }
+  }
+}
+
+}  // namespace dgk

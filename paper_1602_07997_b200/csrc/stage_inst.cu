@@ -2,6 +2,7 @@
 // Exposes the kernel entry points of kernels.cuh for that pair to dg_api.cu through a C getter.
 #include "kernels.cuh"
 #include "tc3_kernels.cuh"
+#include "epk_kernels.cuh"
 
 #if !defined(DG_MODEL) || !defined(DG_N)
 #error "compile with -DDG_MODEL=0|1 -DDG_N=1..10"
@@ -67,3 +68,32 @@ extern "C" int DG_CAT3(dgk_prof_read_, DG_MODEL, DG_N)(long long *out) {
   return (int)cudaMemcpyFromSymbol(out, dgk::dg_prof_buf, sizeof(dgk::dg_prof_buf));
 }
 #endif
+
+// element-per-thread kernel (epk_kernels.cuh): acoustic N = 1, 2 and elastic N = 1; NULL otherwise
+#define DG_HAS_EPK (DG_N == 1 || (DG_N == 2 && DG_MODEL == 0))
+extern "C" const void *DG_CAT3(dgk_get_epk_kernel_, DG_MODEL, DG_N)(int mode) {
+#if DG_HAS_EPK
+  if (mode == dgk::MODE_RHS) return (const void *)&dgk::epk_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
+  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::epk_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
+#endif
+  (void)mode;
+  return nullptr;
+}
+// uploads the reference operators into this translation unit's constant memory: D [3][Np][Np], L [Np][4Nfp] row-major,
+// nbrnode [4][24][Nfp]; fmask [4][Nfp] must equal the kernel's compile-time table.  Returns 0, a cudaError_t, or -1
+// if the face masks differ.
+extern "C" int DG_CAT3(dgk_epk_upload_, DG_MODEL, DG_N)(const float *D, const float *L, const unsigned short *nbrnode, const int *fmask) {
+#if DG_HAS_EPK
+  using Dg = dgk::Deg<DG_N>;
+  constexpr dgk::EpkFmask<DG_N> FM{};
+  for (int i = 0; i < 4 * Dg::NFP; ++i)
+    if (fmask[i] != FM.v[i]) return -1;
+  cudaError_t e = cudaMemcpyToSymbol(dgk::c_epk_D, D, sizeof(float) * 3 * Dg::NP * Dg::NP);
+  if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_epk_L, L, sizeof(float) * Dg::NP * Dg::NFACE);
+  if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_epk_nbrnode, nbrnode, sizeof(unsigned short) * 4 * 24 * Dg::NFP);
+  return (int)e;
+#else
+  (void)D; (void)L; (void)nbrnode; (void)fmask;
+  return -2;
+#endif
+}

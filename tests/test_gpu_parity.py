@@ -35,7 +35,9 @@ def test_rhs_parity_all_degrees(dg, variant, model, N):
     random discontinuous materials, free top + rigid walls.  variant 1 = fused FP32 SIMT kernel,
     variant 4 = pipelined tcgen05 kernel (BF16x3 split, every degree)."""
     case = Case(dg, _sweep_case(model, N), variant=variant)
-    assert case.ctx.variant_name.startswith("simt_fused" if variant == 1 else "tc_pipe")
+    # variant 1 = the SIMT family: element-per-thread kernel for acoustic N <= 2 / elastic N = 1, fused node-per-thread above
+    epk = N == 1 or (N == 2 and model == W.ACOUSTIC)
+    assert case.ctx.variant_name.startswith(("simt_elem_per_thread" if epk else "simt_fused") if variant == 1 else "tc_pipe")
     q32 = case.initial_fields32()
     got = case.gpu_rhs(torch, q32)
     want = case.oracle_rhs(q32.astype(np.float64))
@@ -46,10 +48,13 @@ def test_rhs_parity_all_degrees(dg, variant, model, N):
     assert max(per_field) <= 2 * RHS_TOL, per_field
 
 
-@pytest.mark.parametrize("model,N,E,G", [(W.ACOUSTIC, 2, 1, 5), (W.ACOUSTIC, 3, 8, 3), (W.ACOUSTIC, 4, 2, 1),
-                                         (W.ELASTIC, 2, 4, 7), (W.ELASTIC, 3, 1, 2), (W.ELASTIC, 5, 4, 1)])
+@pytest.mark.parametrize("model,N,E,G", [(W.ACOUSTIC, 1, 1, 16), (W.ACOUSTIC, 2, 1, 5), (W.ACOUSTIC, 3, 8, 3), (W.ACOUSTIC, 4, 2, 1),
+                                         (W.ELASTIC, 1, 2, 8), (W.ELASTIC, 2, 4, 7), (W.ELASTIC, 3, 1, 2), (W.ELASTIC, 5, 4, 1)])
 def test_rhs_parity_other_launch_shapes(dg, model, N, E, G):
-    case = Case(dg, _sweep_case(model, N), elems_per_thread=E, groups_per_cta=G)
+    """An explicit launch shape selects the fused node-per-thread kernel at every degree (also where auto would take the
+    element-per-thread kernel)."""
+    case = Case(dg, _sweep_case(model, N), variant=1, elems_per_thread=E, groups_per_cta=G)
+    assert case.ctx.variant_name.startswith("simt_fused")
     q32 = case.initial_fields32()
     err = rel_l2(case.gpu_rhs(torch, q32), case.oracle_rhs(q32.astype(np.float64)))
     assert err <= RHS_TOL, (case.ctx.variant_name, err)
@@ -232,11 +237,11 @@ def test_padded_private_layout_paths(dg):
 
 
 def test_variant_selection_and_errors(dg):
-    """auto picks the SIMT kernel at N = 1 and acoustic N = 2, the tensor-core kernel elsewhere; unknown variants and
-    misaligned device buffers are rejected."""
+    """auto picks the element-per-thread SIMT kernel at N = 1 and acoustic N = 2, the tensor-core kernel elsewhere;
+    unknown variants and misaligned device buffers are rejected."""
     names = {(m, N): Case(dg, _sweep_case(m, N, n=1)).ctx.variant_name for m in (W.ACOUSTIC, W.ELASTIC) for N in (1, 2, 3)}
-    assert names[(W.ACOUSTIC, 1)].startswith("simt_fused") and names[(W.ELASTIC, 1)].startswith("simt_fused")
-    assert names[(W.ACOUSTIC, 2)].startswith("simt_fused") and names[(W.ELASTIC, 2)].startswith("tc_pipe")
+    assert names[(W.ACOUSTIC, 1)].startswith("simt_elem_per_thread") and names[(W.ELASTIC, 1)].startswith("simt_elem_per_thread")
+    assert names[(W.ACOUSTIC, 2)].startswith("simt_elem_per_thread") and names[(W.ELASTIC, 2)].startswith("tc_pipe")
     assert names[(W.ACOUSTIC, 3)].startswith("tc_pipe") and names[(W.ELASTIC, 3)].startswith("tc_pipe")
     with pytest.raises(dg.DGError):
         Case(dg, _sweep_case(W.ACOUSTIC, 3, n=1), variant=2)
