@@ -57,10 +57,13 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
   if (k >= p.K) return;
 
   // ---- per-element constants and fields
+  // the element's record: G[9], materials, 4 face records -- whole in registers for the acoustic model (32 values),
+  // the first 16 for the elastic one (its face records are read through L1 when needed: register pressure)
+  constexpr int NGL = MODEL == 0 ? NGEO : 16;
   const float *g = p.geo + (size_t)k * NGEO;
-  float gl[16];                                                        // G[9], material constants
+  float gl[NGL];
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
+  for (int i = 0; i < NGL / 4; ++i) {
     const float4 v = __ldg(reinterpret_cast<const float4 *>(g) + i);
     gl[4 * i] = v.x; gl[4 * i + 1] = v.y; gl[4 * i + 2] = v.z; gl[4 * i + 3] = v.w;
   }
@@ -167,10 +170,20 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
     constexpr int FO = MODEL == 0 ? 12 : 16, FS = MODEL == 0 ? 5 : 8;
     float fg[8];
 #pragma unroll
-    for (int i = 0; i < FS; ++i) fg[i] = __ldg(g + FO + FS * f + i);
+    for (int i = 0; i < FS; ++i) fg[i] = MODEL == 0 ? gl[(FO + FS * f + i) % NGL] : __ldg(g + FO + FS * f + i);
     const float nx = fg[0], ny = fg[1], nz = fg[2];
     const int nb = __ldg(p.nbr + (size_t)k * 4 + f);
     const int code = (int)__ldg(p.fcode + (size_t)k * 4 + f);
+    // N = 1: a field of the neighbour is one 16-byte vector (Np = 4): fetch it whole and pick the node afterwards
+    // (a third of the gather instructions; the kernel is bound by the L1/LSU pipe, the ALUs are idle)
+    constexpr bool VGATHER = NP == 4 && MODEL == 0;              // (elastic N = 1: nine vectors per face cost more registers than they save)
+    float4 nq[VGATHER ? NF : 1];
+    if (VGATHER && nb >= 0) {
+      const float4 *src = reinterpret_cast<const float4 *>(p.q_in + (size_t)nb * NV);
+#pragma unroll
+      for (int c = 0; c < NF; ++c) nq[c] = __ldg(src + c);
+    }
+    auto pick = [](const float4 &v, int nn) { return (nn & 2) ? ((nn & 1) ? v.w : v.z) : ((nn & 1) ? v.y : v.x); };
 #pragma unroll
     for (int i = 0; i < NFP; ++i) {
       const int j = f * NFP + i;
@@ -182,9 +195,17 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
         float dp, dvn;
         if (nb >= 0) {
           const int nn = c_epk_nbrnode[(f * 24 + code) * NFP + i];
-          const float *qp = p.q_in + (size_t)nb * NV + nn;
-          dp = __ldg(qp) - um[0];
-          dvn = (__ldg(qp + NP) - um[1]) * nx + (__ldg(qp + 2 * NP) - um[2]) * ny + (__ldg(qp + 3 * NP) - um[3]) * nz;
+          float up[4];
+          if (VGATHER) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) up[c] = pick(nq[c], nn);
+          } else {
+            const float *qp = p.q_in + (size_t)nb * NV + nn;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) up[c] = __ldg(qp + c * NP);
+          }
+          dp = up[0] - um[0];
+          dvn = (up[1] - um[1]) * nx + (up[2] - um[2]) * ny + (up[3] - um[3]) * nz;
         } else {
           acoustic_boundary_jump(nb, um[0], um[1] * nx + um[2] * ny + um[3] * nz, dp, dvn);
         }
@@ -196,10 +217,15 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
         float dv[3], dT[3];
         if (nb >= 0) {
           const int nn = c_epk_nbrnode[(f * 24 + code) * NFP + i];
-          const float *qp = p.q_in + (size_t)nb * NV + nn;
           float up[NF];
+          if (VGATHER) {
 #pragma unroll
-          for (int c = 0; c < NF; ++c) up[c] = __ldg(qp + c * NP);
+            for (int c = 0; c < NF; ++c) up[c] = pick(nq[c], nn);
+          } else {
+            const float *qp = p.q_in + (size_t)nb * NV + nn;
+#pragma unroll
+            for (int c = 0; c < NF; ++c) up[c] = __ldg(qp + c * NP);
+          }
           float Tpx, Tpy, Tpz;
           traction(up, nx, ny, nz, Tpx, Tpy, Tpz);
           dv[0] = up[0] - um[0]; dv[1] = up[1] - um[1]; dv[2] = up[2] - um[2];
