@@ -545,15 +545,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         const int fs = fc % NFL, fuse = fc / NFL;
         constexpr int KPC = C::FCH / 16;                              // k-steps per flux chunk
         if (h % KPC == 0) T3_WAIT(flFull(fs), fuse & 1, 2);
-        const int j0 = 16 * h + 8 * half;
         const float *fl = s_flux + fs * (128 * C::FLS) + r * C::FLS + 16 * (h % KPC) + 8 * half;
         float a[8];
         if (valid) {
           const float4 v0 = *reinterpret_cast<const float4 *>(fl);
           const float4 v1 = *reinterpret_cast<const float4 *>(fl + 4);
+          // (columns beyond 4 Nfp hold zeros or finite penalty terms of an earlier chunk: the operator rows there are zero)
           a[0] = v0.x; a[1] = v0.y; a[2] = v0.z; a[3] = v0.w; a[4] = v1.x; a[5] = v1.y; a[6] = v1.z; a[7] = v1.w;
-#pragma unroll
-          for (int t = 0; t < 8; ++t) a[t] = (j0 + t < NFACE) ? a[t] : 0.f;
         } else {
 #pragma unroll
           for (int t = 0; t < 8; ++t) a[t] = 0.f;
@@ -571,6 +569,10 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     // =================================================== flux warps: rows a4 + a5, one 16-face-node chunk at a time
     const int ft = tid - 384;                           // 0 .. 32 T3_FLUXW - 1
     constexpr int TPT = C::TPT;
+    // the ring starts out zeroed: slots are never fully overwritten (face-node padding, ragged batches), and what the
+    // producers read there must at least be finite
+    for (int x = ft; x < NFL * 128 * C::FLS; x += T3_FLUXW * 32) s_flux[x] = 0.f;
+    tc::named_bar_sync(1, T3_FLUXW * 32);
     int it = 0, fc = 0;
     for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
