@@ -94,6 +94,7 @@ struct T3 {
   static constexpr int TPT = (EB * FCH + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
   static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
   static_assert(NA >= 3, "A ring too small");
+  static_assert((T3_FLUXW * 32) % FCH == 0, "a flux thread keeps its face node across its tasks");
   static_assert(SMEM <= 227 * 1024, "shared memory");
   static_assert(SLOT % 16 == 0 && BSTAGE % 16 == 0, "bulk copy alignment");
 };
@@ -587,23 +588,27 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #pragma unroll 1
       for (int h = 0; h < C::NHC; ++h, ++fc) {
         const int fs = fc % NFL, fuse = fc / NFL;
-        // ---- gather the exterior traces of this thread's tasks (all loads in flight before the first use)
+        // ---- this thread's tasks of the chunk: one face node jj of the chunk, elements e0, e0 + EPI, ... (the face, the
+        // interior node and the row of the neighbour-node table are the same for all of them)
+        constexpr int EPI = T3_FLUXW * 32 / C::FCH;   // element stride between a thread's tasks
+        const int jj = ft % C::FCH, e0 = ft / C::FCH, j = C::FCH * h + jj;
+        const bool jvalid = j < NFACE;
+        const int f = jvalid ? j / NFP : 0;
+        const int nm = jvalid ? (int)__ldg(p.fmask + j) : 0;
+        const unsigned short *nbrow = p.nbrnode + (f * 24) * NFP + (j - f * NFP);
+        // ---- gather the exterior traces (all loads in flight before the first use)
         float ext[TPT][NF];
         int cn[TPT];                                   // packed connectivity of the task's face; INT_MIN = no task
 #pragma unroll
         for (int i = 0; i < TPT; ++i) {
-          const int t = ft + T3_FLUXW * 32 * i;
-          const int e = t / C::FCH, j = C::FCH * h + (t % C::FCH);
+          const int e = e0 + EPI * i;
           cn[i] = (int)0x80000000;
-#pragma unroll
-          for (int c = 0; c < NF; ++c) ext[i][c] = 0.f;
-          if (e < nvalid && j < NFACE) {
-            const int f = j / NFP;
+          if (jvalid && e < nvalid) {
             const int c4 = s_conn[e * 4 + f];
             cn[i] = c4;
             if (c4 >= 0) {
               const int nb = c4 >> 5;
-              const int nn = __ldg(p.nbrnode + (f * 24 + (c4 & 31)) * NFP + (j - f * NFP));
+              const int nn = __ldg(nbrow + (c4 & 31) * NFP);
               const unsigned rel = (unsigned)(nb - k0);
               if (TILE && rel < (unsigned)nvalid) {    // neighbour inside the batch: its values are in the tile
                 const float *qp = s_q + (rel * NF) * PT + nn;
@@ -623,11 +628,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #pragma unroll
         for (int i = 0; i < TPT; ++i) {
           if (cn[i] == (int)0x80000000) continue;
-          const int t = ft + T3_FLUXW * 32 * i;
-          const int e = t / C::FCH, jj = t % C::FCH, j = C::FCH * h + jj;
-          const int f = j / NFP;
+          const int e = e0 + EPI * i;
           const float *g = s_geo + e * NGEO;
-          const int nm = __ldg(p.fmask + j);
           float um[NF];
           if (TILE) {
             const float *qm = s_q + (e * NF) * PT + nm;
