@@ -249,7 +249,9 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
   const StageParams &p = P.s;
 
   extern __shared__ unsigned char smem_raw[];
-  unsigned char *sm = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  // 1024-byte aligned base (swizzled TMA boxes).  Pointer arithmetic on the __shared__ array, not an integer round trip:
+  // the compiler then knows the address space and emits LDS / STS with 32-bit addresses instead of generic LD / ST
+  unsigned char *sm = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
   unsigned char *sB = sm + C::OFF_B;                               // [NB][3][2][NCH][8] bf16
   float *s_flux = reinterpret_cast<float *>(sm + C::OFF_FLUX);     // [NFL][128][FLS] penalty-term chunks
   float *s_scr = reinterpret_cast<float *>(sm + C::OFF_SCR);       // epilogue staging (see the epilogue)
