@@ -13,14 +13,18 @@
 //
 //   * a loader warp streams the batch's field tile, geometric records and packed connectivity into a
 //     double-buffered shared-memory slot with bulk async copies (one batch ahead) and prefetches the batch's
-//     residual into L2 for the epilogue;
-//   * the flux warps (face gather a4 + penalty a5) work through a ring of 16-face-node chunks, several
-//     chunks -- and, with two tile slots, one batch -- ahead of the producers; exterior traces of neighbours
-//     inside the batch come from the shared-memory tile, the others from L2; all gathers of a chunk are
-//     issued before the first use;
+//     residual into L2 for the epilogue; where the tile does not fit in shared memory (N >= 8) it streams the
+//     fields as 2-D TMA boxes of 16 nodes x 128 rows through a ring instead;
+//   * the flux warps (face gather a4 + penalty a5) work through a ring of chunks of 16 (N <= 4) or 32 face nodes,
+//     several chunks -- and, with two tile slots, one batch -- ahead of the producers; exterior traces of
+//     neighbours inside the batch come from the shared-memory tile, the others from L2; all gathers of a chunk
+//     are issued before the first use;
+//   * the epilogue moves chunks of 32 rows x 16|32 nodes as swizzled 2-D TMA boxes (res / q in two chunks ahead,
+//     results out through the same staging buffers) and updates in the TMEM-native layout (thread = row);
+//   * every array the kernel touches has 16-byte aligned rows (pitch PT = Np rounded up to 4; dg_api.cu keeps
+//     padded private copies of the state where Np % 4 != 0);
 //   * degrees whose panel exceeds the TMEM budget (N >= 9) split the output nodes over NSPLIT = 2 CTAs
-//     (each CTA owns half of the operator rows and its own accumulators); degrees whose field tile does not
-//     fit in shared memory (N = 10) let the producers and flux warps read q through L1 instead.
+//     (each CTA owns half of the operator rows and its own accumulators).
 //
 // Warp roles (736 threads): 0-3 epilogue, 4-11 producers (lane = row; tcgen05.st into the TMEM A ring),
 // 12-19 flux, 20 operator stream (cp.async.bulk ring), 21 MMA issue + TMEM allocation, 22 tile loader.
