@@ -250,3 +250,27 @@ def test_variant_selection_and_errors(dg):
     out = torch.zeros_like(buf)
     with pytest.raises(dg.DGError):                                  # q not 16-byte aligned
         case.ctx.rhs(buf.data_ptr() + 4, out.data_ptr())
+
+
+@pytest.mark.parametrize("model,N", [(W.ACOUSTIC, 1), (W.ACOUSTIC, 2), (W.ELASTIC, 1)])
+def test_element_per_thread_kernel_many_ctas(dg, model, N):
+    """The element-per-thread kernel (auto at these degrees) on a mesh of K = 162 000 elements (1 266 CTAs, ragged last
+    one): r_k on sampled elements against the oracle, and one LSRK step stays finite with non-increasing energy."""
+    from oracle import timestep
+    w = W.config(4, N=N, model=model, n=30)
+    w.ic = "random"
+    K = w.K
+    rng = np.random.default_rng(N)
+    sample = np.unique(np.concatenate([np.arange(8), np.arange(K - 8, K), rng.integers(0, K, 48)]))
+    case = Case(dg, w, only_elems=sample)
+    assert case.ctx.variant_name.startswith("simt_elem_per_thread")
+    q32 = case.initial_fields32()
+    got = case.gpu_rhs(torch, q32)[sample]
+    want = case.oracle_rhs(q32.astype(np.float64), sample)
+    assert rel_l2(got, want) <= RHS_TOL, rel_l2(got, want)
+    out = case.gpu_run(torch, q32, case.dt32(), 1)
+    assert np.isfinite(out).all()
+    energy = timestep.energy_acoustic if model == W.ACOUSTIC else timestep.energy_elastic
+    e0 = energy(case.ref, case.mesh, *case.mats, q32.astype(np.float64))
+    e1 = energy(case.ref, case.mesh, *case.mats, out.astype(np.float64))
+    assert 0 < e1 <= e0 * (1 + 1e-6), (e0, e1)
