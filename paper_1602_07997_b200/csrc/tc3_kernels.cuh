@@ -101,6 +101,9 @@ struct T3 {
   static_assert((T3_FLUXW * 32) % FCH == 0, "a flux thread keeps its face node across its tasks");
   static_assert(SMEM <= 227 * 1024, "shared memory");
   static_assert(SLOT % 16 == 0 && BSTAGE % 16 == 0, "bulk copy alignment");
+  static_assert(OFF_SCR % (CW == 32 ? 1024 : 512) == 0 && (32 * CW * 4) % (CW == 32 ? 1024 : 512) == 0,
+                "swizzled TMA staging buffers: 1024-byte (128 B swizzle) / 512-byte (64 B swizzle) alignment");
+  static_assert(OFF_U % 512 == 0 && T3_UCH % 512 == 0, "field chunk ring: 64 B swizzle atoms are 512 bytes");
 };
 
 // Optional role timeline (build with -DDG_PROF): every warp accumulates the cycles it spends in each kind of
