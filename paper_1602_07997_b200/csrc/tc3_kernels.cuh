@@ -95,6 +95,9 @@ struct T3 {
   static constexpr int OFF_SLOT = OFF_U + URING;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
   static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 1024;  // + slack for the 1024-byte alignment (swizzled TMA boxes)
+  // exterior traces of neighbours inside the batch are read from the shared-memory tile (elastic; acoustic from N = 6): at
+  // acoustic N <= 5 the uniform all-L2 gather is faster than the divergent two-path one (measured, C2 0.573 -> 0.564 ms)
+  static constexpr bool INBATCH = TILE && (MODEL == 1 || N >= 6);
   static constexpr int TPT = (EB * FCH + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
   static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
   static_assert(NA >= 3, "A ring too small");
@@ -619,7 +622,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
               const int nb = c4 >> 5;
               const int nn = __ldg(nbrow + (c4 & 31) * NFP);
               const unsigned rel = (unsigned)(nb - k0);
-              if (TILE && rel < (unsigned)nvalid) {    // neighbour inside the batch: its values are in the tile
+              if (C::INBATCH && rel < (unsigned)nvalid) {    // neighbour inside the batch: its values are in the tile
                 const float *qp = s_q + (rel * NF) * PT + nn;
 #pragma unroll
                 for (int c = 0; c < NF; ++c) ext[i][c] = qp[c * PT];
