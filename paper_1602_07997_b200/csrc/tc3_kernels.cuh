@@ -15,7 +15,7 @@
 //     double-buffered shared-memory slot with bulk async copies (one batch ahead) and prefetches the batch's
 //     residual into L2 for the epilogue; where the tile does not fit in shared memory (N >= 8) it streams the
 //     fields as 2-D TMA boxes of 16 nodes x 128 rows through a ring instead;
-//   * the flux warps (face gather a4 + penalty a5) work through a ring of chunks of 16 (N <= 4) or 32 face nodes,
+//   * the flux warps (face gather a4 + penalty a5) work through a ring of chunks of 16 (N <= 3) or 32 face nodes,
 //     several chunks -- and, with two tile slots, one batch -- ahead of the producers; exterior traces of
 //     neighbours inside the batch come from the shared-memory tile, the others from L2; all gathers of a chunk
 //     are issued before the first use;
@@ -60,9 +60,10 @@ struct T3 {
   static constexpr int NSPLIT = NC > 176 ? 2 : 1;              // CTAs sharing one batch (output-node halves)
   static constexpr int NCH = NC / NSPLIT;                      // MMA N of one CTA
   static constexpr int NB = NCH >= 144 ? 3 : 4;                // operator ring stages (shared memory)
-  // flux chunks: 32 face nodes (two k-steps; four tasks in flight per flux thread) from N = 5 up, 16 below, where a
-  // batch has only two to four k-steps of face nodes (measured: N = 3 is 14 % slower with 32, N = 10 9 % faster)
-  static constexpr int FCH = N >= 5 ? 32 : 16;
+  // flux chunks: 32 face nodes (two k-steps; four tasks in flight per flux thread) from N = 4 up, 16 below, where a
+  // batch has only two or three k-steps of face nodes (same-box A/B: N = 3 is 7 % slower with 32, acoustic N = 4 6 %
+  // faster, N = 10 9 % faster)
+  static constexpr int FCH = N >= 4 ? 32 : 16;
   static constexpr int FLS = FCH + 4;                          // floats per row of a chunk (80 / 144-byte rows: conflict-free float4)
   static constexpr int NFL = FCH == 16 ? 4 : (NC >= 176 ? 4 : 3);                // flux chunk ring stages: enough to cover the producers' volume phase
   static constexpr int NG = (NP + 15) / 16;                    // node chunks of 16
