@@ -90,8 +90,16 @@ class ClockSampler:
                                           "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            t0 = time.time()                 # nvidia-smi can take longer to start than the timed region lasts
+            while not self.rows and time.time() - t0 < 10.0 and self.proc.poll() is None:
+                time.sleep(0.01)
         except OSError:
             self.proc = None
+        self.first = 0
+
+    def mark(self):
+        """Start of the timed region: earlier rows are dropped (the last one is kept as a fallback)."""
+        self.first = len(self.rows)
 
     def _read(self):
         for line in self.proc.stdout:
@@ -105,7 +113,8 @@ class ClockSampler:
         self.t.join(timeout=2)
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        rows = self.rows[self.first:] or self.rows[-1:]
+        for r in rows:
             try:
                 sm.append(float(r[0])); mx.append(float(r[1]))
             except (ValueError, IndexError):
@@ -234,10 +243,12 @@ def run_ours(a):
     sptr = stream.cuda_stream
 
     # ---- device-resident timing
+    sampler = ClockSampler(local) if rank == 0 else None      # returns once nvidia-smi delivers rows
     for _ in range(a.warmup):
         ctx.step(d_q.data_ptr(), dt, sptr)
     barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.mark()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record(stream)
     ctx.run(d_q.data_ptr(), dt, a.steps, sptr)
