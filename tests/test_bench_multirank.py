@@ -45,3 +45,28 @@ def test_single_rank_needs_no_process_group():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.max_over_ranks([1.5, 2.5], "cpu", 1) == [1.5, 2.5]
+
+
+def test_clock_sampler_waits_for_a_slow_nvidia_smi(tmp_path, monkeypatch):
+    """The timed region of the default run lasts ~30 ms; the sampler must already deliver rows when it starts and must
+    report only rows from `mark()` on (falling back to the last earlier row rather than to nothing)."""
+    import os
+    import stat
+    import time
+    import bench
+    fake = tmp_path / "nvidia-smi"
+    fake.write_text("#!/bin/bash\nsleep 0.4\ni=0\nwhile true; do i=$((i+1)); if [ $i -le 3 ]; then c=1000; else c=1965; fi\n"
+                    "echo \"$c, 1965, 400.0, Not Active, Not Active, Not Active, Active\"; sleep 0.02; done\n")
+    fake.chmod(fake.stat().st_mode | stat.S_IEXEC)
+    monkeypatch.setenv("PATH", f"{tmp_path}{os.pathsep}{os.environ['PATH']}")
+    s = bench.ClockSampler(0)
+    assert s.rows, "constructor returns only once rows arrive"
+    time.sleep(0.15)                       # "warm-up": the three 1000 MHz rows
+    s.mark()
+    time.sleep(0.1)
+    c = s.stop()
+    assert c["samples"] >= 2 and c["sm_mhz"] == 1965.0 and c["sm_max_mhz"] == 1965.0 and c["reasons"] == ["sw_power_cap"]
+    s = bench.ClockSampler(0)
+    s.mark()
+    s.first += 1000                        # no row inside the region: the last earlier row stands in
+    assert s.stop()["samples"] == 1
