@@ -96,9 +96,10 @@ struct T3 {
   static constexpr int OFF_SLOT = OFF_U + URING;
   static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
   static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 1024;  // + slack for the 1024-byte alignment (swizzled TMA boxes)
-  // exterior traces of neighbours inside the batch are read from the shared-memory tile (elastic; acoustic from N = 6): at
-  // acoustic N <= 5 the uniform all-L2 gather is faster than the divergent two-path one (measured, C2 0.573 -> 0.564 ms)
-  static constexpr bool INBATCH = TILE && (MODEL == 1 || N >= 6);
+  // exterior traces of neighbours inside the batch are read from the shared-memory tile (elastic from N = 3, acoustic from
+  // N = 6): below, the uniform all-L2 gather is faster than the divergent two-path one (same-box A/B: C2 0.573 -> 0.564 ms,
+  // elastic N = 2 2.87 -> 2.81 ms; elastic N = 3..5 are 1-2 % slower without the shared-memory path)
+  static constexpr bool INBATCH = TILE && (MODEL == 1 ? N >= 3 : N >= 6);
   static constexpr int TPT = (EB * FCH + T3_FLUXW * 32 - 1) / (T3_FLUXW * 32);           // flux tasks per thread and chunk
   static_assert(NR <= 128 && NCH <= 256 && NCH % 16 == 0, "one M tile, legal MMA N");
   static_assert(NA >= 3, "A ring too small");
