@@ -12,9 +12,13 @@
  * Conventions:
  *   reference tetrahedron {r,s,t >= -1, r+s+t <= -1}; local vertices v1=(-1,-1,-1), v2=(1,-1,-1),
  *   v3=(-1,1,-1), v4=(-1,-1,1) in the order of `etov`; faces f0:(v1,v2,v3) f1:(v1,v2,v4)
- *   f2:(v2,v3,v4) f3:(v1,v3,v4).  Elements with negative Jacobian have their last two vertices
- *   swapped at create time (this also swaps which faces the `bc` columns 0/1 and 2/3... refer to:
- *   `bc` is indexed AFTER the swap, i.e. give positively oriented elements when tags matter).
+ *   f2:(v2,v3,v4) f3:(v1,v3,v4).  `etov` may list an element's vertices in any order and with
+ *   either orientation.  `bc[k][f]` always refers to face f of element k IN THE CALLER'S vertex
+ *   order (the face opposite the caller's vertex 3, 2, 0, 1 for f = 0..3).  Internally an element
+ *   with negative Jacobian has its last two vertices swapped at create time, which exchanges its
+ *   faces 0 and 1; the library exchanges the two tags with them, so the caller never pre-swaps
+ *   anything.  dg_node_coords, dg_geometry and dg_connectivity report the library's (swapped)
+ *   vertex order: for such an element bctag / nrm / fscale columns 0 and 1 are the caller's 1 and 0.
  *   Nodes: Np=(N+1)(N+2)(N+3)/6 warp-and-blend nodes in lattice order, t slowest,
  *   then s, r fastest; dg_node_coords returns their physical coordinates.
  *   Field layout of q, rhs (DEVICE memory, caller-owned): [K][Nfields][Np] float, node index
@@ -23,9 +27,13 @@
  *
  * Ownership: host arrays passed to dg_create are only read during the call.  The context owns
  * all device constants (operators, geometric factors, connectivity) and scratch (residual,
- * ping-pong state, AB3 history); dg_destroy frees them.  No allocation after dg_create.
+ * ping-pong state, AB3 history); dg_destroy frees them.  No device allocation after dg_create
+ * (the tensor-core variant keeps a host-side cache of TMA descriptors for up to 64 caller
+ * buffers, least recently used evicted; the library's own buffers are encoded at dg_create).
  * dg_rhs/dg_step/dg_run/dg_ab3_step are asynchronous on `cuda_stream` (a cudaStream_t passed as
- * void*, NULL = default stream) and never synchronise the host.
+ * void*, NULL = default stream; it must belong to the context's device) and never synchronise
+ * the host.  Every entry point selects the context's device for the duration of the call and
+ * restores the caller's current device before it returns (dg_create included).
  *
  * Errors: every int function returns 0 on success or a negative DG_ERR_* code; the message is
  * available from dg_last_error() (thread-local).  No exception crosses the boundary.
@@ -77,6 +85,9 @@ typedef struct {
                                  Any other value: DG_ERR_ARG                                           */
   int elems_per_thread;       /* 0 = auto; register blocking E of the SIMT kernel (1..8)         */
   int groups_per_cta;         /* 0 = auto; node groups G per CTA (CTA handles G*E elements)      */
+  int max_ctas;               /* 0 = auto (one persistent CTA per SM); > 0 caps the grid of the
+                                 tensor-core variant so that small test meshes give every CTA
+                                 several batches (tests); < 0: DG_ERR_ARG                         */
 } dg_options;
 
 /* Build a context: reference operators for degree N (1..10), geometric factors, connectivity,
@@ -103,6 +114,11 @@ int dg_rhs(dg_ctx *ctx, const float *d_q, float *d_rhs, void *cuda_stream);
 int dg_step(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);
 /* nsteps LSRK steps in place on d_q (5*nsteps fused stage kernels, one copy if that is odd)     */
 int dg_run(dg_ctx *ctx, float *d_q, float dt, int nsteps, void *cuda_stream);
+/* ONE low-storage stage with explicit coefficients, out of place (the building block of dg_run, exposed for
+ * per-stage control: sampled full-size parity checks, multi-rate drivers):
+ *   res <- a res + dt r(q_in);  q_out <- q_in + b res     (res is the context's residual array; a = 0 ignores it).
+ * d_q_in is not modified; d_q_in == d_q_out is an error (neighbours read the stage input).                     */
+int dg_stage(dg_ctx *ctx, const float *d_q_in, float *d_q_out, float a, float b, float dt, void *cuda_stream);
 /* one AB3 step of PAPER.md eq. (4) in place on d_q; the context keeps r^{m-1}, r^{m-2}
  * (zero after dg_create / dg_ab3_reset, i.e. the first two steps are lower order)               */
 int dg_ab3_step(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);

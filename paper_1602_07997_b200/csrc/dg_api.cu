@@ -113,7 +113,13 @@ struct dg_ctx {
   int epi_cw = 0;                                // tc3: epilogue chunk width (TMA box columns)
   int PT = 0;                                    // tc3: row pitch (floats) of the arrays the kernel works on, Np rounded up to 4
   float *d_qa = nullptr;                         // tc3, PT != Np: padded private copies of the state (d_qa and d_q2 ping-pong)
-  std::map<const void *, std::array<CUtensorMap, 3>> tmaps;   // device array -> descriptors (epilogue boxes of height 32 / Nf EB - 96; field chunks)
+  // device array -> TMA descriptors (epilogue boxes of height 32 / Nf EB - 96; field chunks).  Library-owned buffers are
+  // encoded at dg_create and pinned; caller buffers are encoded on first sight (host-side work only, no device
+  // allocation) and the oldest unpinned entry is evicted beyond TMAP_CACHE entries
+  struct TmapEntry { std::array<CUtensorMap, 3> m; bool pinned; uint64_t stamp; };
+  std::map<const void *, TmapEntry> tmaps;
+  uint64_t tmap_clock = 0;
+  int max_ctas = 0;                              // dg_options.max_ctas: cap on the persistent grid (tests; 0 = one CTA per SM)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;
   // launch configuration
@@ -127,6 +133,19 @@ struct dg_ctx {
 
 namespace {
 
+// Every device entry point runs on the context's device and leaves the caller's current device as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
 template <class T>
 T *upload(const std::vector<T> &h) {
   T *d = nullptr;
@@ -137,7 +156,7 @@ T *upload(const std::vector<T> &h) {
 
 void free_device(dg_ctx *c) {
   if (c->device < 0) return;
-  cudaSetDevice(c->device);
+  DeviceGuard guard(c->device);
   cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_qa); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
@@ -303,9 +322,14 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-const std::array<CUtensorMap, 3> &tensor_maps(dg_ctx *c, const void *ptr) {
+constexpr size_t TMAP_CACHE = 64;
+// returns the descriptors BY VALUE: a later lookup may evict the entry (references into the map dangled)
+std::array<CUtensorMap, 3> tensor_maps(dg_ctx *c, const void *ptr, bool pin = false) {
   auto it = c->tmaps.find(ptr);
-  if (it != c->tmaps.end()) return it->second;
+  if (it != c->tmaps.end()) {
+    it->second.stamp = ++c->tmap_clock;
+    return it->second.m;
+  }
   static encode_tiled_fn encode = nullptr;
   if (!encode) {
     void *fn = nullptr;
@@ -314,7 +338,12 @@ const std::array<CUtensorMap, 3> &tensor_maps(dg_ctx *c, const void *ptr) {
       throw std::runtime_error("cuda: cuTensorMapEncodeTiled is not available");
     encode = (encode_tiled_fn)fn;
   }
-  if (c->tmaps.size() > 32) c->tmaps.clear();
+  if (c->tmaps.size() >= TMAP_CACHE) {           // evict the least recently used caller buffer (never a pinned one)
+    auto victim = c->tmaps.end();
+    for (auto jt = c->tmaps.begin(); jt != c->tmaps.end(); ++jt)
+      if (!jt->second.pinned && (victim == c->tmaps.end() || jt->second.stamp < victim->second.stamp)) victim = jt;
+    if (victim != c->tmaps.end()) c->tmaps.erase(victim);
+  }
   std::array<CUtensorMap, 3> m;
   const int EB = TC3_INFO[c->model][c->N](1);
   const int rlast = c->NF * EB - 96;
@@ -328,7 +357,8 @@ const std::array<CUtensorMap, 3> &tensor_maps(dg_ctx *c, const void *ptr) {
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) throw std::runtime_error("cuda: cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
   }
-  return c->tmaps.emplace(ptr, m).first->second;
+  c->tmaps.emplace(ptr, dg_ctx::TmapEntry{m, pin, ++c->tmap_clock});
+  return m;
 }
 
 int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out, float *rhs, float a, float b, float dt,
@@ -350,7 +380,7 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
     tp3.nbatch = c->nbatch;
     {
       try {
-        const auto &mi = tensor_maps(c, q_in), &mr = tensor_maps(c, c->d_res), &mo = tensor_maps(c, q_out ? q_out : rhs);
+        const auto mi = tensor_maps(c, q_in), mr = tensor_maps(c, c->d_res), mo = tensor_maps(c, q_out ? q_out : rhs);
         for (int h = 0; h < 2; ++h) { tp3.tm_in[h] = mi[h]; tp3.tm_res[h] = mr[h]; tp3.tm_out[h] = mo[h]; }
         tp3.tm_u = mi[2];
       } catch (const std::exception &e) {
@@ -369,6 +399,11 @@ int check_device_ctx(const dg_ctx *c) {
   if (c->device < 0) return fail(DG_ERR_CUDA, "host-only context: no device entry point is available (no CPU fallback)");
   return DG_OK;
 }
+
+#define DG_ENTER_DEVICE(c)                                \
+  if (int e_ = check_device_ctx(c)) return e_;            \
+  DeviceGuard guard_((c)->device);                        \
+  if (!guard_.ok) return fail(DG_ERR_CUDA, "cuda: cannot select the context's device")
 
 }  // namespace
 
@@ -394,6 +429,8 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
     c->NF = model == DG_ACOUSTIC ? 4 : 9;
     c->K = mesh->K;
     c->device = opts ? opts->device : 0;
+    c->max_ctas = opts ? opts->max_ctas : 0;
+    if (c->max_ctas < 0) throw std::invalid_argument("max_ctas must be >= 0");
     for (int64_t k = 0; k < c->K; ++k) {
       const double rho = mat->rho[k], cp = mat->c_or_vp[k];
       if (!(rho > 0.0) || !(cp > 0.0) || !std::isfinite(rho) || !std::isfinite(cp)) {
@@ -416,7 +453,8 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
     c->cmax.assign(mat->c_or_vp, mat->c_or_vp + c->K);
     choose_variant(c, opts);
     if (c->device >= 0) {
-      CUDA_TRY(cudaSetDevice(c->device));
+      DeviceGuard guard(c->device);              // dg_create leaves the caller's current device unchanged
+      if (!guard.ok) throw std::runtime_error("cuda: cannot select device " + std::to_string(c->device));
       const int Np = c->Np, Nfp = c->Nfp;
       std::vector<float> DT((size_t)3 * Np * Np), LT((size_t)4 * Nfp * Np);
       const std::vector<double> *Dm[3] = {&c->ref.Dr, &c->ref.Ds, &c->ref.Dt};
@@ -461,7 +499,9 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
           conn[i] = c->mesh.nbr[i] >= 0 ? (int)(((uint32_t)c->mesh.nbr[i] << 5) | (c->mesh.fcode[i] & 31u)) : -(int)c->mesh.bctag[i];
         c->d_conn = upload(conn);
         CUDA_TRY(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device));
-        c->grid = nsplit * std::max(1, std::min(c->nbatch, c->num_sms / nsplit));   // persistent: one CTA per SM
+        int workers = std::max(1, std::min(c->nbatch, c->num_sms / nsplit));        // persistent: one CTA per SM
+        if (c->max_ctas > 0) workers = std::max(1, std::min(workers, c->max_ctas / nsplit));
+        c->grid = nsplit * workers;
       }
       const size_t nq = (size_t)c->K * c->NF * Np;
       // the tensor-core kernel works on rows of pitch PT (16-byte aligned); when PT != Np the state lives in padded private
@@ -479,6 +519,13 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         CUDA_TRY(cudaMemset(h, 0, nq * sizeof(float)));
       }
       CUDA_TRY(cudaMemset(c->d_res, 0, nqp * sizeof(float)));
+      if (c->tc3) {                              // descriptors of the library's own buffers: encoded once, never evicted
+        tensor_maps(c, c->d_res, true);
+        tensor_maps(c, c->d_q2, true);
+        if (c->d_qa) tensor_maps(c, c->d_qa, true);
+        if (c->PT == Np)
+          for (float *h : c->d_hist) tensor_maps(c, h, true);
+      }
       CUDA_TRY(cudaFuncSetAttribute(c->k_rhs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
       CUDA_TRY(cudaFuncSetAttribute(c->k_stage, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
       CUDA_TRY(cudaDeviceSynchronize());
@@ -611,7 +658,7 @@ static int eval_rhs(dg_ctx *c, const float *d_q, float *d_out, cudaStream_t st, 
 }
 
 int dg_rhs(dg_ctx *c, const float *d_q, float *d_rhs, void *stream) {
-  if (int e = check_device_ctx(c)) return e;
+  DG_ENTER_DEVICE(c);
   if (!d_q || !d_rhs) return fail(DG_ERR_ARG, "NULL device pointer");
   if (d_q == d_rhs) return fail(DG_ERR_ARG, "dg_rhs: d_q and d_rhs must differ");
   c->last_launches = 0;
@@ -619,7 +666,7 @@ int dg_rhs(dg_ctx *c, const float *d_q, float *d_rhs, void *stream) {
 }
 
 int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
-  if (int e = check_device_ctx(c)) return e;
+  DG_ENTER_DEVICE(c);
   if (!d_q || nsteps < 0) return fail(DG_ERR_ARG, "bad argument");
   cudaStream_t st = (cudaStream_t)stream;
   int launches = 0;
@@ -657,8 +704,23 @@ int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
 
 int dg_step(dg_ctx *c, float *d_q, float dt, void *stream) { return dg_run(c, d_q, dt, 1, stream); }
 
+int dg_stage(dg_ctx *c, const float *d_q_in, float *d_q_out, float a, float b, float dt, void *stream) {
+  DG_ENTER_DEVICE(c);
+  if (!d_q_in || !d_q_out) return fail(DG_ERR_ARG, "NULL device pointer");
+  if (d_q_in == d_q_out) return fail(DG_ERR_ARG, "dg_stage: d_q_in and d_q_out must differ (neighbours read the stage input)");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!padded(c)) {
+    c->last_launches = 1;
+    return launch_stage(c, c->k_stage, d_q_in, d_q_out, nullptr, a, b, dt, st);
+  }
+  if (int e = copy_rows(c, c->d_qa, c->PT, d_q_in, c->Np, st)) return e;
+  if (int e = launch_stage(c, c->k_stage, c->d_qa, c->d_q2, nullptr, a, b, dt, st)) return e;
+  c->last_launches = 3;
+  return copy_rows(c, d_q_out, c->Np, c->d_q2, c->PT, st);
+}
+
 int dg_ab3_reset(dg_ctx *c, void *stream) {
-  if (int e = check_device_ctx(c)) return e;
+  DG_ENTER_DEVICE(c);
   const size_t nq = (size_t)c->K * c->NF * c->Np;
   for (float *h : c->d_hist)
     if (cudaMemsetAsync(h, 0, nq * sizeof(float), (cudaStream_t)stream) != cudaSuccess) return fail(DG_ERR_CUDA, "cuda: memset failed");
@@ -667,7 +729,7 @@ int dg_ab3_reset(dg_ctx *c, void *stream) {
 }
 
 int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) {
-  if (int e = check_device_ctx(c)) return e;
+  DG_ENTER_DEVICE(c);
   if (!d_q) return fail(DG_ERR_ARG, "NULL device pointer");
   cudaStream_t st = (cudaStream_t)stream;
   // rotate history: r0 <- new, r1, r2 older (Table 1: R_0, R_-1, R_-2)

@@ -30,11 +30,12 @@ class _Materials(C.Structure):
 
 
 class _Options(C.Structure):
-    _fields_ = [("device", C.c_int), ("variant", C.c_int), ("elems_per_thread", C.c_int), ("groups_per_cta", C.c_int)]
+    _fields_ = [("device", C.c_int), ("variant", C.c_int), ("elems_per_thread", C.c_int), ("groups_per_cta", C.c_int),
+                ("max_ctas", C.c_int)]
 
 
 EXPORTS = ["dg_create", "dg_destroy", "dg_num_fields", "dg_np", "dg_nfp", "dg_num_elements", "dg_node_coords",
-           "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_ab3_step", "dg_ab3_reset", "dg_last_launch_count",
+           "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_stage", "dg_ab3_step", "dg_ab3_reset", "dg_last_launch_count",
            "dg_variant_name", "dg_reference_operators", "dg_geometry", "dg_connectivity", "dg_last_error"]
 
 _lib.dg_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(_Materials), C.POINTER(_Options)]
@@ -51,6 +52,7 @@ _lib.dg_stable_dt.restype = C.c_double
 _lib.dg_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.dg_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
 _lib.dg_run.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int, C.c_void_p]
+_lib.dg_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
 _lib.dg_ab3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
 _lib.dg_ab3_reset.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dg_variant_name.argtypes = [C.c_void_p]
@@ -84,7 +86,7 @@ class Context:
     """dg_create / dg_destroy pair.  Host arrays are numpy; device buffers are raw pointers (ints)."""
 
     def __init__(self, vxyz, etov, N: int, model: int, rho, c_or_vp, vs=None, bc=None, device: int = 0,
-                 elems_per_thread: int = 0, groups_per_cta: int = 0, variant: int = 0):
+                 elems_per_thread: int = 0, groups_per_cta: int = 0, variant: int = 0, max_ctas: int = 0):
         vxyz = np.ascontiguousarray(vxyz, dtype=np.float64)
         etov = np.ascontiguousarray(etov, dtype=np.int32)
         bc = None if bc is None else np.ascontiguousarray(bc, dtype=np.int8)
@@ -93,7 +95,7 @@ class Context:
         vs = None if vs is None else np.ascontiguousarray(vs, dtype=np.float64)
         mesh = _Mesh(vxyz.shape[0], etov.shape[0], _ptr(vxyz), _ptr(etov), _ptr(bc))
         mat = _Materials(_ptr(rho), _ptr(c_or_vp), _ptr(vs))
-        opt = _Options(device, variant, elems_per_thread, groups_per_cta)
+        opt = _Options(device, variant, elems_per_thread, groups_per_cta, max_ctas)
         h = C.c_void_p()
         self._h = None
         _check(_lib.dg_create(C.byref(h), C.byref(mesh), int(N), int(model), C.byref(mat), C.byref(opt)))
@@ -173,6 +175,10 @@ class Context:
 
     def run(self, d_q: int, dt: float, nsteps: int, stream: int | None = None):
         _check(_lib.dg_run(self._h, C.c_void_p(d_q), C.c_float(dt), int(nsteps), C.c_void_p(stream or 0)))
+
+    def stage(self, d_q_in: int, d_q_out: int, a: float, b: float, dt: float, stream: int | None = None):
+        _check(_lib.dg_stage(self._h, C.c_void_p(d_q_in), C.c_void_p(d_q_out), C.c_float(a), C.c_float(b), C.c_float(dt),
+                             C.c_void_p(stream or 0)))
 
     def ab3_step(self, d_q: int, dt: float, stream: int | None = None):
         _check(_lib.dg_ab3_step(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))

@@ -24,6 +24,27 @@ def rel_l2(a, b):
     return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
 
 
+def describe(got, want):
+    """rel-L2 plus where the worst entry is: "rel-L2 3.1e-07, max |err| 2.4e-06 at (element, field, node) = (17, 2, 5)
+    (got ..., want ...), worst element 17 (rel-L2 1.2e-06)" -- so that a failing parity assertion localises the defect."""
+    got = np.asarray(got, dtype=np.float64)
+    want = np.asarray(want, dtype=np.float64)
+    d = np.abs(got - want)
+    idx = np.unravel_index(int(np.argmax(d)), d.shape)
+    per_elem = np.sqrt((d.reshape(d.shape[0], -1) ** 2).sum(axis=1))
+    k = int(np.argmax(per_elem))
+    scale = max(float(np.linalg.norm(want.ravel())), 1e-300)
+    return (f"rel-L2 {rel_l2(got, want):.3e}, max |err| {d[idx]:.3e} at (element, field, node) = {tuple(int(i) for i in idx)} "
+            f"(got {got[idx]:.9g}, want {want[idx]:.9g}), worst element {k} carries {per_elem[k] / scale:.3e} of the rel-L2")
+
+
+def assert_close(got, want, tol, what=""):
+    assert np.isfinite(np.asarray(got)).all(), f"{what}: non-finite values in the GPU result"
+    err = rel_l2(got, want)
+    assert err <= tol, f"{what}: {describe(got, want)} > tolerance {tol:g}"
+    return err
+
+
 class Case:
     """One workload on both sides.  `only_elems` limits the oracle's connectivity to sampled elements."""
 
@@ -56,6 +77,14 @@ class Case:
         self.ctx.rhs(d_q.data_ptr(), d_r.data_ptr(), torch.cuda.current_stream().cuda_stream)
         torch.cuda.synchronize()
         return d_r.cpu().numpy()
+
+    def gpu_stage(self, torch, q32, a, b, dt, d_in=None):
+        """One low-storage stage through dg_stage: returns (q_out as numpy, the device tensor of q_out)."""
+        d_q = torch.from_numpy(np.ascontiguousarray(q32)).cuda() if d_in is None else d_in
+        d_o = torch.full_like(d_q, float("nan"))
+        self.ctx.stage(d_q.data_ptr(), d_o.data_ptr(), a, b, dt, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        return d_o.cpu().numpy(), d_o
 
     def gpu_run(self, torch, q32, dt, nsteps):
         d_q = torch.from_numpy(np.ascontiguousarray(q32)).cuda()

@@ -1,0 +1,229 @@
+"""GPU parity of the LSRK stage mode (row a7 fused into the stage kernels): libdg through the C ABI against the
+fp64 oracle, at every degree on the kernel `auto` picks, with persistent CTAs that loop over several batches, and at
+BASELINE.json's full sizes on sampled elements through the one-stage entry point dg_stage.
+
+Tolerances: BASELINE.json north_star -- rel-L2 <= 2e-6 per RHS evaluation, <= 1e-4 after the LSRK run; a single LSRK
+step (five evaluations, q = q0 + O(dt r)) must agree to 2e-6 in q as well.
+"""
+import re
+
+import numpy as np
+import pytest
+
+from oracle import timestep
+from paper_1602_07997_b200 import workloads as W
+
+from gpu_common import RHS_TOL, RUN_TOL, Case, assert_close, describe, rel_l2
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+A, B = timestep.LSRK_A, timestep.LSRK_B
+
+
+@pytest.fixture(scope="module")
+def dg():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_1602_07997_b200 import dg as mod          # raises if libdg.so is missing: no fallback
+    return mod
+
+
+def _sweep_case(model, N, n=3):
+    w = W.config(4, N=N, model=model, n=n)
+    w.jitter, w.top, w.ic = 0.08, W.BC_FREE, "random"
+    return w
+
+
+def _increment_error(got, want, before):
+    """Error of the step's increment relative to the increment's norm, after discounting what storing q in fp32 costs:
+    |got - want| <= tol |want - before| + 2^-23 |want|.  Returns the left-over as a multiple of |want - before|.
+    (On the pulse workloads the increment of p in stage 2 is below one ulp of p: the storage rounding alone is 2e-4 of the
+    increment's norm there, while a wrong A_s / B_s / residual carry is O(1) of it.)"""
+    got, want, before = (np.asarray(a, dtype=np.float64) for a in (got, want, before))
+    err = np.linalg.norm((got - want).ravel()) - 2.0 ** -23 * np.linalg.norm(want.ravel())
+    return max(err, 0.0) / max(np.linalg.norm((want - before).ravel()), 1e-300)
+
+
+def _info(name, key):
+    m = re.search(key + r"=(\d+)", name)
+    return int(m.group(1)) if m else None
+
+
+# ---------------------------------------------------------------- LSRK trajectory, every degree, the kernel auto picks
+@pytest.mark.parametrize("N", range(1, 11))
+@pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
+def test_run_parity_every_degree_auto(dg, model, N):
+    """dg_run against oracle.timestep.lsrk_run for N = 1..10, both models, on the variant dg_create picks by itself
+    (element-per-thread SIMT kernel at N = 1 and acoustic N = 2, tensor-core kernel elsewhere): one step to 2e-6,
+    three steps to 1e-4.  K = 162, random fields, random discontinuous materials, free top."""
+    case = Case(dg, _sweep_case(model, N))
+    q32 = case.initial_fields32()
+    q64 = q32.astype(np.float64)
+    dt = case.dt32()
+    one = case.gpu_run(torch, q32, dt, 1)
+    want1 = case.oracle_run(q64, dt, 1)
+    assert_close(one, want1, RHS_TOL, f"{case.ctx.variant_name}: one LSRK step")
+    # the increment of the step is what the five stages computed: a wrong A_s / B_s / residual carry shows here at O(1)
+    inc = _increment_error(one, want1, q64)
+    assert inc <= 2e-5, f"{case.ctx.variant_name}: increment of one step off by {inc:.3e}; {describe(one, want1)}"
+    three = case.gpu_run(torch, q32, dt, 3)
+    assert_close(three, case.oracle_run(q64, dt, 3), RUN_TOL, f"{case.ctx.variant_name}: three LSRK steps")
+
+
+# ---------------------------------------------------------------- persistent CTAs over several batches (tensor-core kernel)
+@pytest.mark.parametrize("N", range(1, 11))
+@pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
+def test_stage_parity_several_batches_per_cta(dg, model, N):
+    """The tensor-core kernel with its grid capped (dg_options.max_ctas) so that every persistent CTA works through
+    >= 3 batches, the last one ragged: exercises the double-buffered tile slots, the alternating accumulator sets, the
+    phase wrap of every mbarrier ring, the epilogue's two-chunks-ahead TMA prefetch across batch boundaries and the L2
+    prefetch of the residual -- the paths the kernel takes at full size -- against the full oracle (RHS mode and two LSRK
+    steps)."""
+    w = _sweep_case(model, N)
+    probe = Case(dg, w, variant=4)
+    nsplit = _info(probe.ctx.variant_name, "nsplit")
+    eb = _info(probe.ctx.variant_name, "elems/batch")
+    probe.ctx.close()
+    case = Case(dg, w, variant=4, max_ctas=2 * nsplit)
+    K = case.ctx.K
+    nbatch = -(-K // eb)
+    assert nbatch // 2 >= 3 and K % eb != 0, (K, eb)          # >= 3 batches per CTA and a ragged last batch
+    q32 = case.initial_fields32()
+    q64 = q32.astype(np.float64)
+    assert_close(case.gpu_rhs(torch, q32), case.oracle_rhs(q64), RHS_TOL, f"{case.ctx.variant_name}: r(q), {nbatch} batches on 2 workers")
+    dt = case.dt32()
+    got = case.gpu_run(torch, q32, dt, 2)
+    want = case.oracle_run(q64, dt, 2)
+    assert_close(got, want, 1e-5, f"{case.ctx.variant_name}: two LSRK steps, {nbatch} batches on 2 workers")
+    # one worker (pair): every batch of the mesh on the same CTA
+    one = Case(dg, w, variant=4, max_ctas=nsplit)
+    assert np.array_equal(one.gpu_run(torch, q32, dt, 2), got), "result depends on how batches are dealt to CTAs"
+
+
+@pytest.mark.parametrize("model,N,n,steps", [(W.ACOUSTIC, 3, 14, 2), (W.ACOUSTIC, 5, 14, 2), (W.ELASTIC, 3, 11, 2), (W.ELASTIC, 7, 11, 1)])
+def test_stage_parity_natural_grid_three_batches_per_cta(dg, model, N, n, steps):
+    """The same with the grid the library launches by itself (one CTA per SM): meshes large enough that each of the 148
+    persistent CTAs gets >= 3 batches (acoustic K = 16 464 > 148 x 32 x 3; elastic K = 7 986 > 148 x 14 x 3), full oracle."""
+    w = _sweep_case(model, N, n=n)
+    case = Case(dg, w)
+    assert case.ctx.variant_name.startswith("tc_pipe")
+    eb = _info(case.ctx.variant_name, "elems/batch")
+    assert -(-case.ctx.K // eb) >= 3 * 148
+    q32 = case.initial_fields32()
+    dt = case.dt32()
+    got = case.gpu_run(torch, q32, dt, steps)
+    want = case.oracle_run(q32.astype(np.float64), dt, steps)
+    assert_close(got, want, 1e-5, f"{case.ctx.variant_name}: {steps} LSRK step(s) on K = {case.ctx.K}")
+
+
+# ---------------------------------------------------------------- full size: one stage at a time on sampled elements
+def _sample(K, eb, rng, nrand=160):
+    """First / last elements, one element of each of ~nrand evenly spread batches (so that every region of the batch
+    sequence -- and with it every persistent CTA's early, middle and late batches -- is hit) and random ones."""
+    nb = -(-K // eb)
+    spread = (np.linspace(0, nb - 1, min(nb, nrand)).astype(np.int64) * eb + rng.integers(0, eb, min(nb, nrand))).clip(0, K - 1)
+    return np.unique(np.concatenate([np.arange(8), np.arange(K - 8, K), spread, rng.integers(0, K, 64)]))
+
+
+def _two_stages_sampled(dg, w, sample_extra=None, **opts):
+    """Stage 1 (A_1 = 0) and stage 2 (carries the residual) of the LSRK step through dg_stage on the full mesh; the
+    oracle evaluates r_k on the sampled elements from the same global state:
+        q1 = q0 + B_1 dt r(q0);   q2 = q1 + B_2 (A_2 dt r(q0) + dt r(q1))."""
+    K = w.K
+    rng = np.random.default_rng(w.N + 17 * w.model)
+    probe = dg.from_workload(W.config(4, N=w.N, model=w.model, n=1), device=0, **opts)
+    eb = _info(probe.variant_name, "elems/batch") or 128
+    probe.close()
+    sample = _sample(K, eb, rng)
+    if sample_extra is not None:
+        sample = np.unique(np.concatenate([sample, sample_extra(w)]))
+    case = Case(dg, w, only_elems=sample, **opts)
+    q0 = case.initial_fields32()
+    dt = case.dt32()
+    q1, d_q1 = case.gpu_stage(torch, q0, 0.0, B[0], dt)
+    r0 = case.oracle_rhs(q0.astype(np.float64), sample)
+    want1 = q0[sample].astype(np.float64) + np.float32(B[0]) * np.float64(dt) * r0
+    name = case.ctx.variant_name
+    assert_close(q1[sample], want1, RHS_TOL, f"{name}: stage 1 on {len(sample)} sampled elements of K = {K}")
+    inc1 = _increment_error(q1[sample], want1, q0[sample])
+    q2, _ = case.gpu_stage(torch, None, A[1], B[1], dt, d_in=d_q1)
+    r1 = case.oracle_rhs(q1.astype(np.float64), sample)          # from the GPU's own q1: isolates stage 2
+    res2 = np.float32(A[1]) * (np.float64(dt) * r0) + np.float64(dt) * r1
+    want2 = q1[sample].astype(np.float64) + np.float32(B[1]) * res2
+    assert_close(q2[sample], want2, RHS_TOL, f"{name}: stage 2 (residual carried) on sampled elements of K = {K}")
+    inc2 = _increment_error(q2[sample], want2, q1[sample])
+    assert max(inc1, inc2) <= 5e-5, f"{name}: stage increments off by {inc1:.3e} / {inc2:.3e}"
+    # everything outside the sample at least finite, and nothing left unwritten (the output started as NaN)
+    assert np.isfinite(q1).all() and np.isfinite(q2).all()
+    return case
+
+
+def _pulse_support(w):
+    vx, et, bc, cell = w.mesh()
+    cen = vx[et].mean(axis=1)
+    return np.flatnonzero(np.linalg.norm(cen - 0.5, axis=1) < 0.2)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_full_size_stage_mode_sampled(dg, cfg):
+    """BASELINE.json sizes in the launch configuration bench.py times (148 persistent CTAs, 81 / 78 / 40 batches each)."""
+    w = W.config(cfg)
+    _two_stages_sampled(dg, w, sample_extra=_pulse_support if w.ic == "pulse" else None)
+
+
+@pytest.mark.parametrize("model,N", [(W.ACOUSTIC, 1), (W.ACOUSTIC, 2), (W.ELASTIC, 1)])
+def test_element_per_thread_stage_mode_sampled(dg, model, N):
+    """The element-per-thread kernel (auto at these degrees) in stage mode on K = 162 000 elements (1 266 CTAs)."""
+    w = W.config(4, N=N, model=model, n=30)
+    w.ic = "random"
+    case = _two_stages_sampled(dg, w)
+    assert case.ctx.variant_name.startswith("simt_elem_per_thread")
+
+
+# ---------------------------------------------------------------- full size: every element, kernel against kernel
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_full_size_tensor_core_vs_simt_every_element(dg, cfg):
+    """Two LSRK steps at full size on the tensor-core kernel and on the fused FP32 SIMT kernel (oracle-pinned on the small
+    meshes above): every element compared, so a defect confined to batches the sampled tests miss cannot hide."""
+    w = W.config(cfg)
+    a = dg.from_workload(w, device=0, variant=4)
+    xyz = a.node_coords()
+    q32 = w.initial_fields(xyz).astype(np.float32)
+    del xyz
+    dt = float(np.float32(a.stable_dt(0.5)))
+    d_a = torch.from_numpy(q32).cuda()
+    a.run(d_a.data_ptr(), dt, 2)
+    torch.cuda.synchronize()
+    a.close()
+    b = dg.from_workload(w, device=0, variant=1)
+    d_b = torch.from_numpy(q32).cuda()
+    b.run(d_b.data_ptr(), dt, 2)
+    torch.cuda.synchronize()
+    b.close()
+    diff = (d_a - d_b).double()
+    err = float(diff.norm() / d_b.double().norm())
+    worst = int(diff.abs().amax(dim=(1, 2)).argmax())
+    assert err <= 1e-5, f"{w.name}: tensor-core vs SIMT after two steps rel-L2 {err:.3e}, worst element {worst}"
+    inc = float(diff.norm() / (d_b - torch.from_numpy(q32).cuda()).double().norm())
+    assert inc <= 1e-4, f"{w.name}: increments differ by {inc:.3e}, worst element {worst}"
+
+
+@pytest.mark.parametrize("model,N", [(W.ACOUSTIC, 1), (W.ACOUSTIC, 2), (W.ELASTIC, 1)])
+def test_element_per_thread_vs_node_per_thread_every_element(dg, model, N):
+    w = W.config(4, N=N, model=model, n=30)
+    w.ic = "random"
+    out = []
+    for opts in ({}, {"variant": 1, "elems_per_thread": 1}):
+        ctx = dg.from_workload(w, device=0, **opts)
+        if not out:
+            q32 = w.initial_fields(ctx.node_coords()).astype(np.float32)
+            dt = float(np.float32(ctx.stable_dt(0.5)))
+        d = torch.from_numpy(q32).cuda()
+        ctx.run(d.data_ptr(), dt, 2)
+        torch.cuda.synchronize()
+        out.append((ctx.variant_name, d))
+        ctx.close()
+    assert out[0][0].startswith("simt_elem_per_thread") and out[1][0].startswith("simt_fused")
+    err = float((out[0][1] - out[1][1]).double().norm() / out[1][1].double().norm())
+    assert err <= 1e-5, (out[0][0], out[1][0], err)

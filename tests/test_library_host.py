@@ -124,3 +124,45 @@ def test_bad_inputs_are_rejected(dg):
     with pytest.raises(dg.DGError) as e:          # boundary faces tagged "interior"
         dg.Context(vxyz, etov, 2, dg.ACOUSTIC, one, one, None, np.zeros((6, 4), np.int8), device=-1)
     assert e.value.code == -2
+
+
+def test_boundary_tags_follow_the_callers_face_numbering(dg, refelems):
+    """include/dg.h: `bc[k][f]` refers to face f of element k in the CALLER's vertex order, whatever the orientation; the
+    library permutes the tags together with the vertices when it fixes a negative Jacobian.  Every element is given in a
+    random vertex order (half of them negatively oriented) with distinct tags on the cube's top (FREE) and the other
+    walls (RIGID); afterwards every tagged face must carry the tag of the wall its normal points to."""
+    n = 2
+    vxyz, etov, _ = W.kuhn_cube(n, 0.05, seed=1)
+    bc = W.wall_tags(n, etov, top=W.BC_FREE, other=W.BC_RIGID)
+    opp = np.array([3, 2, 0, 1])                     # face f is opposite the local vertex opp[f]
+    face_of_opp = np.argsort(opp)                    # vertex v is opposite face face_of_opp[v]
+    rng = np.random.default_rng(5)
+    et, tags = etov.copy(), bc.copy()
+    for k in range(len(et)):
+        perm = rng.permutation(4)
+        et[k] = etov[k][perm]
+        tags[k] = bc[k][face_of_opp[perm[opp]]]      # new face f = old face opposite the old vertex perm[opp[f]]
+    one = np.ones(len(et))
+    ctx = dg.Context(vxyz, et, 2, dg.ACOUSTIC, one, one, None, tags, device=-1)
+    geo, con = ctx.geometry(), ctx.connectivity()
+    assert np.all(geo["J"] > 0)
+    lib_tags, nrm = con["bctag"], geo["nrm"]
+    assert (lib_tags > 0).sum() == (bc > 0).sum() == 6 * 2 * n * n
+    top = (lib_tags > 0) & (nrm[..., 2] > 0.99)       # boundary faces whose outward normal is +z (walls are planar)
+    assert np.all(lib_tags[top] == W.BC_FREE) and top.sum() == 2 * n * n
+    wall = (lib_tags > 0) & ~top
+    assert np.all(lib_tags[wall] == W.BC_RIGID)
+    assert np.all(np.abs(np.abs(nrm[wall]).max(axis=-1) - 1.0) < 1e-12)       # axis-aligned outward wall normals
+    # and the oracle, given the same permuted input, agrees tag for tag
+    m = omesh.build(refelems(2), vxyz, et, tags)
+    assert np.array_equal(lib_tags, m.bctag)
+    # a caller who "pre-swaps" tags as the old header text suggested would put FREE on a side wall: the library must not
+    wrong = tags.copy()
+    wrong[:, [0, 1]] = wrong[:, [1, 0]]
+    if not np.array_equal(wrong, tags):
+        try:
+            bad = dg.Context(vxyz, et, 2, dg.ACOUSTIC, one, one, None, wrong, device=-1)
+            lt = bad.connectivity()["bctag"]
+            assert not np.all(lt[(lt > 0) & (bad.geometry()["nrm"][..., 2] > 0.99)] == W.BC_FREE)
+        except dg.DGError as e:                      # or the swap leaves a boundary face untagged: also a loud failure
+            assert e.code == -2
