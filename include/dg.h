@@ -119,9 +119,27 @@ int dg_run(dg_ctx *ctx, float *d_q, float dt, int nsteps, void *cuda_stream);
  *   res <- a res + dt r(q_in);  q_out <- q_in + b res     (res is the context's residual array; a = 0 ignores it).
  * d_q_in is not modified; d_q_in == d_q_out is an error (neighbours read the stage input).                     */
 int dg_stage(dg_ctx *ctx, const float *d_q_in, float *d_q_out, float a, float b, float dt, void *cuda_stream);
-/* one AB3 step of PAPER.md eq. (4) in place on d_q; the context keeps r^{m-1}, r^{m-2}
- * (zero after dg_create / dg_ab3_reset, i.e. the first two steps are lower order)               */
+/* ---- hooks for multi-rate (local) time stepping (elements advance with a step that fits
+ * their own size and wave speed; the drivers of refs [16,17,33] are not part of this library).  A driver numbers the
+ * elements level by level (dg_element_dt gives each element's own stable step), then advances one level at a time:
+ * dg_stage_range is dg_stage restricted to the elements k_begin <= k < k_end -- q_out and the residual of every other
+ * element are left untouched, exterior traces are read from d_q_in whatever range the neighbour is in (the driver
+ * keeps / interpolates the coarse levels' states there: "trace buffering").  k_begin and k_end must be multiples of
+ * dg_range_alignment() (k_end may also be K).  Not available where the library pads rows (DG_ERR_ARG).              */
+int dg_element_dt(const dg_ctx *ctx, double cfl, double *dt_host /* [K] */);
+int dg_range_alignment(const dg_ctx *ctx);
+int dg_stage_range(dg_ctx *ctx, const float *d_q_in, float *d_q_out, float a, float b, float dt, int64_t k_begin,
+                   int64_t k_end, void *cuda_stream);
+/* The paper's own time integrator, third-order Adams-Bashforth (eq. (4)):
+ *   q^{m+1} = q^m + dt (23/12 r^m - 16/12 r^{m-1} + 5/12 r^{m-2}),   one evaluation of r per step.
+ * The context keeps r^{m-1}, r^{m-2} (R_-1, R_-2 of Table 1).  Steady state: ONE fused kernel per step
+ * (r(q), the combination and the rotation of the history by pointer); d_q is updated in place (ping-pong inside, one
+ * device copy per call if the number of steps is odd: prefer dg_ab3_run over repeated dg_ab3_step).  Start-up (DESIGN.md
+ * reading Q21 -- the paper does not say how the first two steps are taken): while fewer than two earlier right-hand sides
+ * are on record (after dg_create / dg_ab3_reset) a step is r(q) into the history plus one LSRK(5,4) step, which keeps the
+ * third order.  dt must be the same from step to step (dg_ab3_reset when it changes).                               */
 int dg_ab3_step(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);
+int dg_ab3_run(dg_ctx *ctx, float *d_q, float dt, int nsteps, void *cuda_stream);
 int dg_ab3_reset(dg_ctx *ctx, void *cuda_stream);
 
 /* number of kernels/copies the last dg_rhs/dg_step/dg_run/dg_ab3_step call enqueued             */

@@ -52,11 +52,20 @@ def lsrk_run(q0, dt, nsteps, rhs):
 
 
 def ab3_step(q, r_hist, dt, rhs):
-    """eq. (4): q^{m+1} = q^m + dt sum_s a_s r^{m-s+1}; r_hist = [r^{m-1}, r^{m-2}]."""
+    """eq. (4):  q^{m+1} = q^m + dt (23/12 r^m - 16/12 r^{m-1} + 5/12 r^{m-2}).
+
+    r_hist: the right-hand sides of earlier steps, newest first, at most two; updated in place.
+    Start-up (reading Q21: eq. (4) needs r^{m-1}, r^{m-2}, and the paper does not say how the first two steps
+    are taken): while fewer than two earlier right-hand sides exist the step is one LSRK(5,4) step -- fourth order, so
+    the third order of eq. (4) survives; starting eq. (4) from a zero history instead leaves an O(dt) error that never
+    decays -- and r(q^m) is recorded for the steps that follow."""
     r0 = rhs(q)
-    q += dt * (AB3[0] * r0 + AB3[1] * r_hist[0] + AB3[2] * r_hist[1])
-    r_hist[1] = r_hist[0]
-    r_hist[0] = r0
+    if len(r_hist) < 2:
+        lsrk_step(q, np.zeros_like(q), dt, rhs)
+    else:
+        q += dt * (AB3[0] * r0 + AB3[1] * r_hist[0] + AB3[2] * r_hist[1])
+    r_hist.insert(0, r0)
+    del r_hist[2:]
     return q
 
 

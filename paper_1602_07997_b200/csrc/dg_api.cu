@@ -74,23 +74,13 @@ const double RK_B[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 136
 }  // namespace
 
 namespace dgk {
-// AB3 update of PAPER.md eq. (4): q += dt (a1 r0 + a2 r1 + a3 r2), pure streaming
-__global__ void ab3_update_kernel(float4 *__restrict__ q, const float4 *__restrict__ r0, const float4 *__restrict__ r1,
-                                  const float4 *__restrict__ r2, size_t n4, float c0, float c1, float c2) {
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
-    float4 a = q[i];
-    const float4 x = r0[i], y = r1[i], z = r2[i];
-    a.x += c0 * x.x + c1 * y.x + c2 * z.x;
-    a.y += c0 * x.y + c1 * y.y + c2 * z.y;
-    a.z += c0 * x.z + c1 * y.z + c2 * z.z;
-    a.w += c0 * x.w + c1 * y.w + c2 * z.w;
-    q[i] = a;
+// rows of `np` floats from pitch `spitch` to pitch `dpitch` (caller layout <-> the tensor-core kernel's padded rows)
+__global__ void repitch_kernel(float *__restrict__ dst, int dpitch, const float *__restrict__ src, int spitch, int np, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t r = i / (unsigned)np;
+    const int c = (int)(i - r * (unsigned)np);
+    dst[r * dpitch + c] = src[r * spitch + c];
   }
-}
-__global__ void ab3_update_tail_kernel(float *__restrict__ q, const float *__restrict__ r0, const float *__restrict__ r1,
-                                       const float *__restrict__ r2, size_t begin, size_t n, float c0, float c1, float c2) {
-  const size_t i = begin + (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) q[i] += c0 * r0[i] + c1 * r1[i] + c2 * r2[i];
 }
 
 }  // namespace dgk
@@ -116,14 +106,15 @@ struct dg_ctx {
   // device array -> TMA descriptors (epilogue boxes of height 32 / Nf EB - 96; field chunks).  Library-owned buffers are
   // encoded at dg_create and pinned; caller buffers are encoded on first sight (host-side work only, no device
   // allocation) and the oldest unpinned entry is evicted beyond TMAP_CACHE entries
-  struct TmapEntry { std::array<CUtensorMap, 3> m; bool pinned; uint64_t stamp; };
+  struct TmapEntry { std::array<CUtensorMap, 5> m; bool pinned; uint64_t stamp; };
   std::map<const void *, TmapEntry> tmaps;
   uint64_t tmap_clock = 0;
   int max_ctas = 0;                              // dg_options.max_ctas: cap on the persistent grid (tests; 0 = one CTA per SM)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
-  int hist_head = 0;
+  int hist_head = 0;                             // d_hist[hist_head] = r^{m-1}, d_hist[(hist_head + 1) % 3] = r^{m-2}
+  int nhist = 0;                                 // AB3: right-hand sides of earlier steps on record (start-up while < 2)
   // launch configuration
-  const void *k_rhs = nullptr, *k_stage = nullptr;
+  const void *k_rhs = nullptr, *k_stage = nullptr, *k_ab3 = nullptr;
   int E = 0, G = 0, NT = 0, grid = 0;
   size_t smem = 0;
   int nbatch = 0, num_sms = 0;
@@ -263,6 +254,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     c->tc3 = true;
     c->k_rhs = TC3_KERNELS[c->model][c->N](dgk::MODE_RHS);
     c->k_stage = TC3_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    c->k_ab3 = TC3_KERNELS[c->model][c->N](dgk::MODE_AB3);
     const info_getter info = TC3_INFO[c->model][c->N];
     const int EB = info(1);
     c->nbatch = (int)((c->K + EB - 1) / EB);
@@ -283,6 +275,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     c->epk = true;
     c->k_rhs = EPK_KERNELS[c->model][c->N](dgk::MODE_RHS);
     c->k_stage = EPK_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    c->k_ab3 = EPK_KERNELS[c->model][c->N](dgk::MODE_AB3);
     c->NT = 128;
     c->smem = 0;
     c->grid = (int)((c->K + 127) / 128);
@@ -303,7 +296,8 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
   }
   c->k_rhs = KERNELS[c->model][c->N](E, dgk::MODE_RHS);
   c->k_stage = KERNELS[c->model][c->N](E, dgk::MODE_STAGE);
-  if (!c->k_rhs || !c->k_stage) throw std::invalid_argument("elems_per_thread not instantiated for this model");
+  c->k_ab3 = KERNELS[c->model][c->N](E, dgk::MODE_AB3);
+  if (!c->k_rhs || !c->k_stage || !c->k_ab3) throw std::invalid_argument("elems_per_thread not instantiated for this model");
   c->E = E;
   c->G = G;
   c->NT = ((G * Np + 31) / 32) * 32;
@@ -324,7 +318,7 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 constexpr size_t TMAP_CACHE = 64;
 // returns the descriptors BY VALUE: a later lookup may evict the entry (references into the map dangled)
-std::array<CUtensorMap, 3> tensor_maps(dg_ctx *c, const void *ptr, bool pin = false) {
+std::array<CUtensorMap, 5> tensor_maps(dg_ctx *c, const void *ptr, bool pin = false) {
   auto it = c->tmaps.find(ptr);
   if (it != c->tmaps.end()) {
     it->second.stamp = ++c->tmap_clock;
@@ -344,16 +338,21 @@ std::array<CUtensorMap, 3> tensor_maps(dg_ctx *c, const void *ptr, bool pin = fa
       if (!jt->second.pinned && (victim == c->tmaps.end() || jt->second.stamp < victim->second.stamp)) victim = jt;
     if (victim != c->tmaps.end()) c->tmaps.erase(victim);
   }
-  std::array<CUtensorMap, 3> m;
+  std::array<CUtensorMap, 5> m;
   const int EB = TC3_INFO[c->model][c->N](1);
   const int rlast = c->NF * EB - 96;
-  for (int h = 0; h < 3; ++h) {          // [2]: field chunks of 16 nodes x 128 rows for the producers (no-tile configurations)
+  // [0], [1]: epilogue boxes of epi_cw nodes x 32 | rlast rows; [2]: field chunks of 16 nodes x 128 rows for the producers
+  // (no-tile configurations); [3], [4]: the AB3 epilogue's boxes of epi_cw / 2 nodes.  Swizzle = the box's row length
+  for (int h = 0; h < 5; ++h) {
+    const int width = h == 2 ? 16 : (h < 2 ? c->epi_cw : c->epi_cw / 2);
     const cuuint64_t dims[2] = {(cuuint64_t)c->PT, (cuuint64_t)c->K * c->NF};
     const cuuint64_t strides[1] = {(cuuint64_t)c->PT * 4};
-    const cuuint32_t box[2] = {(cuuint32_t)(h == 2 ? 16 : c->epi_cw), (cuuint32_t)(h == 2 ? 128 : (h ? rlast : 32))};
+    const int height = h == 2 ? 128 : ((h == 0 || h == 3) ? 32 : rlast);
+    const cuuint32_t box[2] = {(cuuint32_t)width, (cuuint32_t)height};
     const cuuint32_t es[2] = {1, 1};
+    const CUtensorMapSwizzle swz = width == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : (width == 16 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B);
     const CUresult r = encode(&m[h], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(ptr), dims, strides, box, es,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, (h < 2 && c->epi_cw == 32) ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) throw std::runtime_error("cuda: cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
   }
@@ -361,13 +360,28 @@ std::array<CUtensorMap, 3> tensor_maps(dg_ctx *c, const void *ptr, bool pin = fa
   return m;
 }
 
+// elements per unit of work of the chosen kernel: element ranges of dg_stage_range start on multiples of it
+int range_alignment(const dg_ctx *c) {
+  if (c->tc3) return TC3_INFO[c->model][c->N](1);
+  if (c->epk) return 1;
+  return c->G * c->E;
+}
+
+// AB3 launches (kernel == c->k_ab3): hist1 = r^{m-1}, hist2 = r^{m-2} (inputs), rhs = the buffer that receives r^m
 int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out, float *rhs, float a, float b, float dt,
-                 cudaStream_t st) {
+                 cudaStream_t st, int64_t kbeg = 0, int64_t kend = -1, float *hist1 = nullptr, const float *hist2 = nullptr) {
+  if (kend < 0) kend = c->K;
+  if (kbeg >= kend) return DG_OK;
   dgk::StageParams p;
-  p.q_in = q_in; p.q_out = q_out; p.res = c->d_res; p.rhs = rhs;
+  p.q_in = q_in; p.q_out = q_out; p.res = hist1 ? hist1 : c->d_res; p.rhs = rhs; p.hist2 = hist2;
   p.DT = c->d_DT; p.LT = c->d_LT; p.geo = c->d_geo; p.nbr = c->d_nbr; p.fcode = c->d_fcode;
   p.fmask = c->d_fmask; p.nbrnode = c->d_nbrnode;
-  p.K = (int)c->K; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
+  p.K = (int)kend; p.kbeg = (int)kbeg; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
+  int grid = c->grid;
+  if (kbeg != 0 || kend != c->K) {
+    const int unit = c->epk ? 128 : range_alignment(c);
+    grid = (int)((kend - kbeg + unit - 1) / unit);
+  }
   dgk::Tc3Params tp3;
   void *args[] = {&p};
   if (c->epk && (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15))
@@ -375,21 +389,34 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   if (c->tc3) {
     if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
     tp3.s = p;
+    tp3.s.K = (int)c->K;                          // (the kernel bounds a ragged last batch by the mesh, ranges by batches)
     tp3.Bimg = c->d_Bimg;
     tp3.conn = c->d_conn;
-    tp3.nbatch = c->nbatch;
+    const int EB = range_alignment(c), nsplit = TC3_INFO[c->model][c->N](4);
+    tp3.bbeg = (int)(kbeg / EB);
+    tp3.nbatch = (int)((kend + EB - 1) / EB);
+    int workers = std::max(1, std::min(tp3.nbatch - tp3.bbeg, c->num_sms / nsplit));
+    if (c->max_ctas > 0) workers = std::max(1, std::min(workers, c->max_ctas / nsplit));
+    grid = nsplit * workers;
     {
       try {
-        const auto mi = tensor_maps(c, q_in), mr = tensor_maps(c, c->d_res), mo = tensor_maps(c, q_out ? q_out : rhs);
+        const auto mi = tensor_maps(c, q_in), mr = tensor_maps(c, p.res), mo = tensor_maps(c, q_out ? q_out : rhs);
         for (int h = 0; h < 2; ++h) { tp3.tm_in[h] = mi[h]; tp3.tm_res[h] = mr[h]; tp3.tm_out[h] = mo[h]; }
         tp3.tm_u = mi[2];
+        if (hist2) {
+          const auto m2 = tensor_maps(c, hist2), m0 = tensor_maps(c, rhs);
+          for (int h = 0; h < 2; ++h) {
+            tp3.tm3_in[h] = mi[3 + h]; tp3.tm3_h1[h] = mr[3 + h]; tp3.tm3_h2[h] = m2[3 + h];
+            tp3.tm3_r0[h] = m0[3 + h]; tp3.tm3_out[h] = mo[3 + h];
+          }
+        }
       } catch (const std::exception &e) {
         return fail(DG_ERR_CUDA, e.what());
       }
     }
     args[0] = &tp3;
   }
-  cudaError_t e = cudaLaunchKernel(kernel, dim3(c->grid), dim3(c->NT), args, c->smem, st);
+  cudaError_t e = cudaLaunchKernel(kernel, dim3(grid), dim3(c->NT), args, c->smem, st);
   if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " launching " + c->variant);
   return DG_OK;
 }
@@ -514,20 +541,20 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         CUDA_TRY(cudaMalloc(&c->d_qa, nqp * sizeof(float)));
         CUDA_TRY(cudaMemset(c->d_qa, 0, nqp * sizeof(float)));
       }
-      for (float *&h : c->d_hist) {
-        CUDA_TRY(cudaMalloc(&h, nq * sizeof(float)));
-        CUDA_TRY(cudaMemset(h, 0, nq * sizeof(float)));
+      for (float *&h : c->d_hist) {             // AB3 history, in the kernel's own row pitch
+        CUDA_TRY(cudaMalloc(&h, nqp * sizeof(float)));
+        CUDA_TRY(cudaMemset(h, 0, nqp * sizeof(float)));
       }
       CUDA_TRY(cudaMemset(c->d_res, 0, nqp * sizeof(float)));
       if (c->tc3) {                              // descriptors of the library's own buffers: encoded once, never evicted
         tensor_maps(c, c->d_res, true);
         tensor_maps(c, c->d_q2, true);
         if (c->d_qa) tensor_maps(c, c->d_qa, true);
-        if (c->PT == Np)
-          for (float *h : c->d_hist) tensor_maps(c, h, true);
+        for (float *h : c->d_hist) tensor_maps(c, h, true);
       }
       CUDA_TRY(cudaFuncSetAttribute(c->k_rhs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
       CUDA_TRY(cudaFuncSetAttribute(c->k_stage, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
+      CUDA_TRY(cudaFuncSetAttribute(c->k_ab3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem));
       CUDA_TRY(cudaDeviceSynchronize());
     }
   } catch (const std::invalid_argument &e) {
@@ -640,8 +667,10 @@ int dg_connectivity(const dg_ctx *c, int32_t *elemP, int32_t *nodeP, int8_t *bct
 // caller layout [K Nf][Np] <-> the tensor-core kernel's private layout [K Nf][PT] (pad columns stay zero)
 static bool padded(const dg_ctx *c) { return c->tc3 && c->PT != c->Np; }
 static int copy_rows(dg_ctx *c, float *dst, int dpitch, const float *src, int spitch, cudaStream_t st) {
-  cudaError_t e = cudaMemcpy2DAsync(dst, (size_t)dpitch * 4, src, (size_t)spitch * 4, (size_t)c->Np * 4, (size_t)c->K * c->NF,
-                                    cudaMemcpyDeviceToDevice, st);
+  const size_t n = (size_t)c->K * c->NF * c->Np;
+  const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 32);
+  dgk::repitch_kernel<<<blocks, 256, 0, st>>>(dst, dpitch, src, spitch, c->Np, n);
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " in the layout conversion");
   return DG_OK;
 }
@@ -719,39 +748,86 @@ int dg_stage(dg_ctx *c, const float *d_q_in, float *d_q_out, float a, float b, f
   return copy_rows(c, d_q_out, c->Np, c->d_q2, c->PT, st);
 }
 
+int dg_range_alignment(const dg_ctx *c) { return c ? range_alignment(c) : fail(DG_ERR_ARG, "NULL context"); }
+
+int dg_stage_range(dg_ctx *c, const float *d_q_in, float *d_q_out, float a, float b, float dt, int64_t k_begin, int64_t k_end,
+                   void *stream) {
+  DG_ENTER_DEVICE(c);
+  if (!d_q_in || !d_q_out) return fail(DG_ERR_ARG, "NULL device pointer");
+  if (d_q_in == d_q_out) return fail(DG_ERR_ARG, "dg_stage_range: d_q_in and d_q_out must differ");
+  if (k_begin < 0 || k_end > c->K || k_begin > k_end) return fail(DG_ERR_ARG, "dg_stage_range: need 0 <= k_begin <= k_end <= K");
+  if (k_begin % range_alignment(c) != 0 || (k_end % range_alignment(c) != 0 && k_end != c->K))
+    return fail(DG_ERR_ARG, "dg_stage_range: k_begin and k_end must be multiples of dg_range_alignment() (k_end may be K)");
+  if (padded(c)) return fail(DG_ERR_ARG, "dg_stage_range: not available for degrees whose rows the library pads (N = 2, 4, 8, 10 on the tensor-core variant); create the context with variant = 1");
+  c->last_launches = k_begin < k_end ? 1 : 0;
+  return launch_stage(c, c->k_stage, d_q_in, d_q_out, nullptr, a, b, dt, (cudaStream_t)stream, k_begin, k_end);
+}
+
+int dg_element_dt(const dg_ctx *c, double cfl, double *dt_host) {
+  if (!c || !dt_host || !(cfl > 0.0)) return fail(DG_ERR_ARG, "bad argument");
+  for (int64_t k = 0; k < c->K; ++k) {
+    double fs = 0.0;
+    for (int f = 0; f < 4; ++f) fs = std::max(fs, c->mesh.fscale[4 * k + f]);
+    dt_host[k] = cfl / ((c->N + 1.0) * (c->N + 1.0) * c->cmax[k] * fs);
+  }
+  return DG_OK;
+}
+
 int dg_ab3_reset(dg_ctx *c, void *stream) {
   DG_ENTER_DEVICE(c);
-  const size_t nq = (size_t)c->K * c->NF * c->Np;
-  for (float *h : c->d_hist)
-    if (cudaMemsetAsync(h, 0, nq * sizeof(float), (cudaStream_t)stream) != cudaSuccess) return fail(DG_ERR_CUDA, "cuda: memset failed");
+  (void)stream;
+  c->nhist = 0;                                  // the next two steps are start-up steps again
   c->hist_head = 0;
   return DG_OK;
 }
 
-int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) {
+// nsteps steps of PAPER.md eq. (4).  Steady state: ONE fused kernel per step (r(q), the AB3 combination and the rotation of
+// the history R_0, R_-1, R_-2 of Table 1, by pointer), q ping-pong as in dg_run.  Start-up (DESIGN.md reading
+// Q21): while fewer than two earlier right-hand sides are on record a step is r(q) into the history + one LSRK(5,4) step.
+int dg_ab3_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
   DG_ENTER_DEVICE(c);
-  if (!d_q) return fail(DG_ERR_ARG, "NULL device pointer");
+  if (!d_q || nsteps < 0) return fail(DG_ERR_ARG, "bad argument");
   cudaStream_t st = (cudaStream_t)stream;
-  // rotate history: r0 <- new, r1, r2 older (Table 1: R_0, R_-1, R_-2)
-  c->hist_head = (c->hist_head + 2) % 3;
-  float *r0 = c->d_hist[c->hist_head], *r1 = c->d_hist[(c->hist_head + 1) % 3], *r2 = c->d_hist[(c->hist_head + 2) % 3];
   int launches = 0;
-  if (int e = eval_rhs(c, d_q, r0, st, launches)) return e;
-  const size_t nq = (size_t)c->K * c->NF * c->Np, n4 = nq / 4;
+  c->last_launches = 0;
+  if (nsteps == 0) return DG_OK;
+  float *cur = d_q, *oth = c->d_q2;
+  if (padded(c)) {
+    if (int e = copy_rows(c, c->d_qa, c->PT, d_q, c->Np, st)) return e;
+    cur = c->d_qa;
+    ++launches;
+  }
   const float c0 = dt * (23.f / 12.f), c1 = dt * (-16.f / 12.f), c2 = dt * (5.f / 12.f);
-  if (n4) {
-    const int blocks = (int)std::min<size_t>((n4 + 255) / 256, (size_t)148 * 16);
-    dgk::ab3_update_kernel<<<blocks, 256, 0, st>>>((float4 *)d_q, (const float4 *)r0, (const float4 *)r1, (const float4 *)r2, n4, c0, c1, c2);
+  for (int s = 0; s < nsteps; ++s) {
+    float *h1 = c->d_hist[c->hist_head], *h2 = c->d_hist[(c->hist_head + 1) % 3], *r0 = c->d_hist[(c->hist_head + 2) % 3];
+    if (c->nhist < 2) {
+      if (int e = launch_stage(c, c->k_rhs, cur, nullptr, r0, 0.f, 0.f, 0.f, st)) return e;
+      for (int i = 0; i < 5; ++i) {
+        if (int e = launch_stage(c, c->k_stage, cur, oth, nullptr, (float)RK_A[i], (float)RK_B[i], dt, st)) return e;
+        std::swap(cur, oth);
+      }
+      launches += 6;
+      ++c->nhist;
+    } else {
+      if (int e = launch_stage(c, c->k_ab3, cur, oth, r0, c1, c2, c0, st, 0, -1, h1, h2)) return e;
+      std::swap(cur, oth);
+      ++launches;
+    }
+    c->hist_head = (c->hist_head + 2) % 3;       // r^m becomes r^{m-1}, r^{m-1} becomes r^{m-2}
+  }
+  if (padded(c)) {
+    if (int e = copy_rows(c, d_q, c->Np, cur, c->PT, st)) return e;
+    ++launches;
+  } else if (cur != d_q) {
+    cudaError_t e = cudaMemcpyAsync(d_q, cur, (size_t)c->K * c->NF * c->Np * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e));
     ++launches;
   }
-  if (nq % 4) {
-    dgk::ab3_update_tail_kernel<<<1, 32, 0, st>>>(d_q, r0, r1, r2, n4 * 4, nq, c0, c1, c2);
-    ++launches;
-  }
-  if (cudaGetLastError() != cudaSuccess) return fail(DG_ERR_CUDA, "cuda: AB3 update launch failed");
   c->last_launches = launches;
   return DG_OK;
 }
+
+int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) { return dg_ab3_run(c, d_q, dt, 1, stream); }
 
 #ifdef DG_PROF
 // development builds only (-DDG_PROF): per-warp wait-cycle counters of the last variant-4 launch, [296][23][5] int64

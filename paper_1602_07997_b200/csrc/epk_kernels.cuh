@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
   constexpr int NV = NF * NP;                                          // values per element
   static_assert(NV % 4 == 0, "an element's fields are moved as 16-byte vectors");
   constexpr EpkFmask<N> FM{};
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int k = p.kbeg + blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= p.K) return;
 
   // ---- per-element constants and fields
@@ -250,6 +250,18 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
     float4 *dst = reinterpret_cast<float4 *>(p.rhs + base);
 #pragma unroll
     for (int i = 0; i < NV / 4; ++i) dst[i] = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+  } else if (MODE == MODE_AB3) {
+    float4 *dst = reinterpret_cast<float4 *>(p.rhs + base), *pq = reinterpret_cast<float4 *>(p.q_out + base);
+    const float4 *h1 = reinterpret_cast<const float4 *>(p.res + base), *h2 = reinterpret_cast<const float4 *>(p.hist2 + base);
+#pragma unroll
+    for (int i = 0; i < NV / 4; ++i) {
+      const float4 x = h1[i], y = __ldg(h2 + i);
+      dst[i] = make_float4(r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+      pq[i] = make_float4(fmaf(p.b, y.x, fmaf(p.a, x.x, fmaf(p.dt, r[4 * i], q[4 * i]))),
+                          fmaf(p.b, y.y, fmaf(p.a, x.y, fmaf(p.dt, r[4 * i + 1], q[4 * i + 1]))),
+                          fmaf(p.b, y.z, fmaf(p.a, x.z, fmaf(p.dt, r[4 * i + 2], q[4 * i + 2]))),
+                          fmaf(p.b, y.w, fmaf(p.a, x.w, fmaf(p.dt, r[4 * i + 3], q[4 * i + 3]))));
+    }
   } else {
     float4 *pres = reinterpret_cast<float4 *>(p.res + base), *pq = reinterpret_cast<float4 *>(p.q_out + base);
 #pragma unroll

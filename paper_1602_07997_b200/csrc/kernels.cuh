@@ -17,13 +17,16 @@
 
 namespace dgk {
 
-enum { MODE_RHS = 0, MODE_STAGE = 1 };
+// MODE_AB3: the paper's own update (eq. (4)) as the epilogue: rhs <- r(q_in) (the new r^m),
+// q_out <- q_in + dt r^m + a res + b hist2 with res = r^{m-1}, hist2 = r^{m-2} (read only) and dt, a, b = dt (23, -16, 5) / 12
+enum { MODE_RHS = 0, MODE_STAGE = 1, MODE_AB3 = 2 };
 
 struct StageParams {
   const float *__restrict__ q_in;
   float *__restrict__ q_out;
   float *__restrict__ res;
   float *__restrict__ rhs;
+  const float *__restrict__ hist2;           // MODE_AB3: r^{m-2}
   const float *__restrict__ DT;              // [3][Np][Np]  DT[d][m][n] = D_d[n][m]
   const float *__restrict__ LT;              // [4Nfp][Np]   LT[j][n]    = LIFT[n][j]
   const float *__restrict__ geo;             // [K][GEO_*]
@@ -31,7 +34,8 @@ struct StageParams {
   const unsigned char *__restrict__ fcode;   // [K][4] g*6+s
   const unsigned short *__restrict__ fmask;  // [4Nfp]
   const unsigned short *__restrict__ nbrnode;  // [4][24][Nfp]
-  int K;
+  int K;                                     // end of the element range this launch works on (all elements: K)
+  int kbeg;                                  // first element of the range (dg_stage_range; 0 otherwise)
   int G;                                     // node groups per CTA
   float a, b, dt;                            // LSRK A_s, B_s, dt
 };
@@ -63,7 +67,7 @@ __global__ void stage_kernel(const StageParams p) {
   const int EB = p.G * E;
   const int NT = blockDim.x;
   const int tid = threadIdx.x;
-  const int k0 = blockIdx.x * EB;
+  const int k0 = p.kbeg + blockIdx.x * EB;
   const int nvalid = min(EB, p.K - k0);
 
   extern __shared__ float4 smem4[];
@@ -294,6 +298,9 @@ __global__ void stage_kernel(const StageParams p) {
       const size_t idx = base + (size_t)f * NP;
       if (MODE == MODE_RHS) {
         p.rhs[idx] = r[ee][f];
+      } else if (MODE == MODE_AB3) {
+        p.rhs[idx] = r[ee][f];
+        p.q_out[idx] = fmaf(p.b, __ldg(p.hist2 + idx), fmaf(p.a, p.res[idx], fmaf(p.dt, r[ee][f], s_q[(e * NF + f) * NP + n])));
       } else {
         float rs = p.dt * r[ee][f];
         if (p.a != 0.f) rs = fmaf(p.a, p.res[idx], rs);

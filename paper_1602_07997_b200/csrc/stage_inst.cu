@@ -17,6 +17,7 @@ template <int E>
 const void *pick_mode(int mode) {
   if (mode == dgk::MODE_RHS) return (const void *)&dgk::stage_kernel<DG_MODEL, DG_N, E, dgk::MODE_RHS>;
   if (mode == dgk::MODE_STAGE) return (const void *)&dgk::stage_kernel<DG_MODEL, DG_N, E, dgk::MODE_STAGE>;
+  if (mode == dgk::MODE_AB3) return (const void *)&dgk::stage_kernel<DG_MODEL, DG_N, E, dgk::MODE_AB3>;
   return nullptr;
 }
 }  // namespace
@@ -40,6 +41,7 @@ extern "C" size_t DG_CAT3(dgk_stage_smem_bytes_, DG_MODEL, DG_N)(int EB) { retur
 extern "C" const void *DG_CAT3(dgk_get_tc3_kernel_, DG_MODEL, DG_N)(int mode) {
   if (mode == dgk::MODE_RHS) return (const void *)&dgk::tc3_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
   if (mode == dgk::MODE_STAGE) return (const void *)&dgk::tc3_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
+  if (mode == dgk::MODE_AB3) return (const void *)&dgk::tc3_stage_kernel<DG_MODEL, DG_N, dgk::MODE_AB3>;
   return nullptr;
 }
 // launch geometry: what = 0 shared-memory bytes, 1 elements per batch, 2 NCH, 3 k-steps, 4 NSPLIT, 5 tile staged in
@@ -75,6 +77,7 @@ extern "C" const void *DG_CAT3(dgk_get_epk_kernel_, DG_MODEL, DG_N)(int mode) {
 #if DG_HAS_EPK
   if (mode == dgk::MODE_RHS) return (const void *)&dgk::epk_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
   if (mode == dgk::MODE_STAGE) return (const void *)&dgk::epk_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
+  if (mode == dgk::MODE_AB3) return (const void *)&dgk::epk_stage_kernel<DG_MODEL, DG_N, dgk::MODE_AB3>;
 #endif
   (void)mode;
   return nullptr;

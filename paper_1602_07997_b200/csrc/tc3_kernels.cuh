@@ -82,7 +82,11 @@ struct T3 {
   static constexpr int NES = CW == 16 ? 3 : 2;                 // epilogue staging stages
   static constexpr int SCR = 4 * NES * 2 * 32 * CW * 4;        // per epilogue warp: [stage][res | q][32 rows][CW] floats (swizzled)
   static constexpr int NBAR = 2 * NA + 2 * NB + 2 * NFL + 4 + 4 + 12 + 2 * T3_NU;
-  static constexpr int FIXED = NB * BSTAGE + NFL * FLUX_SLOT + SCR + NBAR * 8 + 16 + 1024;
+  // neighbour-node table [4][24][NFP] and face mask [4 NFP] (uint16) for the flux warps: in shared memory, so that the
+  // exterior-trace gather is one dependent load (connectivity -> address) instead of two through L2 (the L1 left beside
+  // ~210 KB of shared memory does not hold the table: ncu showed 28 % of the flux warps' stall samples on these loads)
+  static constexpr int TAB = ((96 + 4) * NFP * 2 + 15) / 16 * 16;
+  static constexpr int FIXED = NB * BSTAGE + NFL * FLUX_SLOT + SCR + TAB + NBAR * 8 + 16 + 1024;
   static constexpr int TILE_SLOT = TILE_RAW;
   static constexpr bool TILE = FIXED + TILE_SLOT + META <= T3_SMEM_LIMIT;   // field tile staged in shared memory
   static constexpr int NQ = !TILE ? 2 : (FIXED + 2 * (TILE_SLOT + META) <= T3_SMEM_LIMIT ? 2 : 1);
@@ -94,7 +98,8 @@ struct T3 {
   static constexpr int OFF_SCR = OFF_FLUX + NFL * FLUX_SLOT;
   static constexpr int OFF_U = OFF_SCR + SCR;
   static constexpr int OFF_SLOT = OFF_U + URING;
-  static constexpr int OFF_BAR = OFF_SLOT + NQ * SLOT;
+  static constexpr int OFF_TAB = OFF_SLOT + NQ * SLOT;
+  static constexpr int OFF_BAR = OFF_TAB + TAB;
   static constexpr int SMEM = OFF_BAR + NBAR * 8 + 16 + 1024;  // + slack for the 1024-byte alignment (swizzled TMA boxes)
   // exterior traces of neighbours inside the batch are read from the shared-memory tile (elastic from N = 3, acoustic from
   // N = 6): below, the uniform all-L2 gather is faster than the divergent two-path one (same-box A/B: C2 0.573 -> 0.564 ms,
@@ -139,11 +144,15 @@ struct Tc3Params {
   StageParams s;
   const uint16_t *__restrict__ Bimg;   // [NSPLIT][NSTEP][3][2][NCH][8] bf16 operator panel image (host: build_tc3_image)
   const int *__restrict__ conn;        // [K][4] packed connectivity: (neighbour << 5 | face code) or -(bc tag)
-  int nbatch;
+  int nbatch;                          // end of the batch range this launch works on (all batches: ceil(K / EB))
+  int bbeg;                            // first batch of the range (dg_stage_range; 0 otherwise)
   // epilogue TMA descriptors: 2-D views [K Nf rows][PT] of q_in, res and q_out | rhs with
   // boxes of CW nodes x 32 rows ([0]) and CW x (Nf EB - 96) rows ([1], the last row quadrant of an elastic batch)
   CUtensorMap tm_in[2], tm_res[2], tm_out[2];
   CUtensorMap tm_u;                    // q_in, boxes of 16 nodes x 128 rows, 64 B swizzle: the producers' field chunks (no tile)
+  // MODE_AB3 (eq. (4)): boxes of CW / 2 nodes (three inputs per chunk share the staging of two): q_in, r^{m-1} (s.res),
+  // r^{m-2} (s.hist2) in; r^m (s.rhs), q_out out
+  CUtensorMap tm3_in[2], tm3_h1[2], tm3_h2[2], tm3_r0[2], tm3_out[2];
 };
 
 namespace tc {
@@ -164,8 +173,15 @@ template <int NCOL>
 __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t *v) {
   if constexpr (NCOL == 32) {
     tmem_ld32(taddr, v);
+  } else if constexpr (NCOL == 8) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t"
+        "tcgen05.wait::ld.sync.aligned;\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+        : "r"(taddr)
+        : "memory");
   } else {
-    static_assert(NCOL == 16, "16 or 32 columns");
+    static_assert(NCOL == 16, "8, 16 or 32 columns");
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n\t"
         "tcgen05.wait::ld.sync.aligned;\n"
@@ -322,39 +338,51 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     // Chunks of 32 rows x CW output nodes move as 2-D TMA boxes: res / q in two chunks ahead (mbarrier per warp
     // and stage), results out through the same swizzled staging buffers (bulk async-group).  The update runs in
     // the TMEM-native layout (thread = row); the 128 B / 64 B swizzle keeps its float4 accesses conflict-free.
-    constexpr int CW = C::CW;
-    constexpr uint32_t BUFB = 32 * CW * 4;             // bytes of one staging buffer (1024-byte aligned)
+    // MODE_AB3 (the paper's update, eq. (4)) has three inputs per chunk (q, r^{m-1}, r^{m-2}) and two outputs (r^m, q): its
+    // chunks are half as wide, so that three staging buffers per stage fit where the LSRK update keeps two.
+    constexpr bool AB3 = MODE == MODE_AB3;
+    constexpr int CW = AB3 ? C::CW / 2 : C::CW;
+    constexpr int NBUF = AB3 ? 3 : 2;
+    constexpr int LW = CW >= 16 ? 16 : 8;              // columns per TMEM load
+    constexpr uint32_t BUFB = 32 * CW * 4;             // bytes of one staging buffer (aligned to 8 rows of it: the swizzle atom)
     constexpr int RLAST = C::NR - 96;                  // rows of the last quadrant (32 acoustic, 30 elastic)
     const int qd = warp;
     const int hmap = (qd == 3 && RLAST != 32) ? 1 : 0; // which box height
     const uint32_t boxbytes = (uint32_t)((hmap ? RLAST : 32) * CW * 4);
     constexpr int NES = C::NES;
-    unsigned char *bufs = reinterpret_cast<unsigned char *>(s_scr) + warp * (NES * 2 * BUFB);   // [stage][res | q]
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(s_scr) + warp * (NES * 2 * 32 * C::CW * 4);   // [stage][res | q (| r^{m-2})]
     const int n0 = hid * NCH;
     const int ncv = min(NCH, NP - n0);
     const bool need_res = MODE == MODE_STAGE && p.a != 0.f;
     const bool leader = tc::elect_one();               // the same lane issues and retires every TMA operation
     auto issue = [&](int stg, int b, int c0) {         // TMA loads of chunk (b, c0) into stage stg
-      if (MODE == MODE_STAGE && b < P.nbatch && leader) {
+      if (MODE != MODE_RHS && b < P.nbatch && leader) {
         const int row0 = b * EB * NF + qd * 32;
-        const uint32_t dR = tc::smem_u32(bufs + (stg * 2) * BUFB), dQ = dR + BUFB;
-        tc::mbar_expect_tx(epiFull(warp, stg), need_res ? 2 * boxbytes : boxbytes);
-        tc::tma_load_2d(dQ, &P.tm_in[hmap], n0 + c0, row0, epiFull(warp, stg));
-        if (need_res) tc::tma_load_2d(dR, &P.tm_res[hmap], n0 + c0, row0, epiFull(warp, stg));
+        const uint32_t dR = tc::smem_u32(bufs + (stg * NBUF) * BUFB), dQ = dR + BUFB;
+        if (AB3) {
+          tc::mbar_expect_tx(epiFull(warp, stg), 3 * boxbytes);
+          tc::tma_load_2d(dQ, &P.tm3_in[hmap], n0 + c0, row0, epiFull(warp, stg));
+          tc::tma_load_2d(dR, &P.tm3_h1[hmap], n0 + c0, row0, epiFull(warp, stg));
+          tc::tma_load_2d(dQ + BUFB, &P.tm3_h2[hmap], n0 + c0, row0, epiFull(warp, stg));
+        } else {
+          tc::mbar_expect_tx(epiFull(warp, stg), need_res ? 2 * boxbytes : boxbytes);
+          tc::tma_load_2d(dQ, &P.tm_in[hmap], n0 + c0, row0, epiFull(warp, stg));
+          if (need_res) tc::tma_load_2d(dR, &P.tm_res[hmap], n0 + c0, row0, epiFull(warp, stg));
+        }
       }
     };
     auto advance = [&](int &b, int &c0) {
       c0 += CW;
       if (c0 >= ncv) { c0 = 0; b += nworkers; }
     };
-    int ab = worker, ac0 = 0;                          // the chunk two ahead of the current one
+    int ab = P.bbeg + worker, ac0 = 0;                 // the chunk two ahead of the current one
     issue(0, ab, ac0);
     advance(ab, ac0);
     issue(1, ab, ac0);
     advance(ab, ac0);
     int it = -1, stg = 0, astg = 2 % NES, set = 0;     // stage of the current chunk / of the chunk two ahead
     uint32_t par = 0;                                  // phase bit per stage
-    for (int b = worker, c0 = 0; b < P.nbatch; advance(b, c0), stg = (stg + 1 == NES ? 0 : stg + 1)) {
+    for (int b = P.bbeg + worker, c0 = 0; b < P.nbatch; advance(b, c0), stg = (stg + 1 == NES ? 0 : stg + 1)) {
       if (c0 == 0) {
         ++it;
         set = C::NSETS == 2 ? (it & 1) : 0;
@@ -365,11 +393,11 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       float acc[CW];                     // main + small accumulator, summed 16 columns at a time (register pressure)
       {
 #pragma unroll
-        for (int h = 0; h < CW / 16; ++h) {
-          uint32_t vm[16], vs[16];
-          T3_TIMED(2, tc::tmem_ld<16>(t0 + 16 * h, vm); tc::tmem_ld<16>(t0 + NCH + 16 * h, vs));
+        for (int h = 0; h < CW / LW; ++h) {
+          uint32_t vm[LW], vs[LW];
+          T3_TIMED(2, tc::tmem_ld<LW>(t0 + LW * h, vm); tc::tmem_ld<LW>(t0 + NCH + LW * h, vs));
 #pragma unroll
-          for (int j = 0; j < 16; ++j) acc[16 * h + j] = __uint_as_float(vm[j]) + __uint_as_float(vs[j]);
+          for (int j = 0; j < LW; ++j) acc[LW * h + j] = __uint_as_float(vm[j]) + __uint_as_float(vs[j]);
         }
       }
       if (c0 + CW >= ncv) {              // accumulators drained: the MMA warp may start the next batch on this set
@@ -377,13 +405,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         __syncwarp();
         if (lane == 0) tc::mbar_arrive(accEmpty(set));
       }
-      if (MODE == MODE_STAGE) {
+      if (MODE != MODE_RHS) {
         T3_WAIT(epiFull(warp, stg), (par >> stg) & 1, 1);   // this chunk's boxes have landed
         par ^= 1u << stg;
       }
-      unsigned char *bR = bufs + (stg * 2) * BUFB, *bQ = bR + BUFB;
-      // swizzle: 16-byte chunk j4 of row `lane` sits at chunk j4 ^ f(lane) (128B: lane & 7, 64B: (lane >> 1) & 3)
-      const int sw = CW == 32 ? (lane & 7) : ((lane >> 1) & 3);
+      unsigned char *bR = bufs + (stg * NBUF) * BUFB, *bQ = bR + BUFB;
+      // swizzle: 16-byte chunk j4 of row `lane` sits at chunk j4 ^ f(lane) (128B: lane & 7, 64B: (lane >> 1) & 3, 32B: (lane >> 2) & 1)
+      const int sw = CW == 32 ? (lane & 7) : (CW == 16 ? ((lane >> 1) & 3) : ((lane >> 2) & 1));
 #pragma unroll
       for (int j4 = 0; j4 < CW / 4; ++j4) {
         const int off = lane * (CW * 4) + ((j4 ^ sw) << 4);
@@ -393,6 +421,11 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         for (int t = 0; t < 4; ++t) r[t] = acc[4 * j4 + t];
         if (MODE == MODE_RHS) {
           *pr = make_float4(r[0], r[1], r[2], r[3]);
+        } else if (AB3) {                // eq. (4): q += dt (23/12 r^m - 16/12 r^{m-1} + 5/12 r^{m-2}); dt, a, b carry the products
+          const float4 H1 = *pr, Q = *pq, H2 = *reinterpret_cast<const float4 *>(bQ + BUFB + off);
+          *pr = make_float4(r[0], r[1], r[2], r[3]);
+          *pq = make_float4(fmaf(p.b, H2.x, fmaf(p.a, H1.x, fmaf(p.dt, r[0], Q.x))), fmaf(p.b, H2.y, fmaf(p.a, H1.y, fmaf(p.dt, r[1], Q.y))),
+                            fmaf(p.b, H2.z, fmaf(p.a, H1.z, fmaf(p.dt, r[2], Q.z))), fmaf(p.b, H2.w, fmaf(p.a, H1.w, fmaf(p.dt, r[3], Q.w))));
         } else {
           float4 R = make_float4(0.f, 0.f, 0.f, 0.f);
           if (need_res) R = *pr;
@@ -409,6 +442,9 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         const int row0 = b * EB * NF + qd * 32;
         if (MODE == MODE_RHS) {
           tc::tma_store_2d(&P.tm_out[hmap], n0 + c0, row0, tc::smem_u32(bR));
+        } else if (AB3) {
+          tc::tma_store_2d(&P.tm3_r0[hmap], n0 + c0, row0, tc::smem_u32(bR));
+          tc::tma_store_2d(&P.tm3_out[hmap], n0 + c0, row0, tc::smem_u32(bQ));
         } else {
           tc::tma_store_2d(&P.tm_res[hmap], n0 + c0, row0, tc::smem_u32(bR));
           tc::tma_store_2d(&P.tm_out[hmap], n0 + c0, row0, tc::smem_u32(bQ));
@@ -457,7 +493,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       if (++slot == NA) { slot = 0; phase ^= 1; }
     };
     int it = 0, fc = 0, uc = 0;
-    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+    for (int b = P.bbeg + worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
       const bool valid = r < C::NR && e < nvalid;
@@ -587,9 +623,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     // the ring starts out zeroed: slots are never fully overwritten (face-node padding, ragged batches), and what the
     // producers read there must at least be finite
     for (int x = ft; x < NFL * 128 * C::FLS; x += T3_FLUXW * 32) s_flux[x] = 0.f;
+    unsigned short *s_nbrnode = reinterpret_cast<unsigned short *>(sm + C::OFF_TAB);   // [4][24][NFP]
+    unsigned short *s_fmask = s_nbrnode + 96 * NFP;                                    // [4 NFP]
+    for (int x = ft; x < 96 * NFP; x += T3_FLUXW * 32) s_nbrnode[x] = __ldg(p.nbrnode + x);
+    for (int x = ft; x < NFACE; x += T3_FLUXW * 32) s_fmask[x] = __ldg(p.fmask + x);
     tc::named_bar_sync(1, T3_FLUXW * 32);
     int it = 0, fc = 0;
-    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+    for (int b = P.bbeg + worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
       const int qs = it % NQ, quse = it / NQ;
@@ -608,8 +648,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         const int jj = ft % C::FCH, e0 = ft / C::FCH, j = C::FCH * h + jj;
         const bool jvalid = j < NFACE;
         const int f = jvalid ? j / NFP : 0;
-        const int nm = jvalid ? (int)__ldg(p.fmask + j) : 0;
-        const unsigned short *nbrow = p.nbrnode + (f * 24) * NFP + (j - f * NFP);
+        const int nm = jvalid ? (int)s_fmask[j] : 0;
+        const unsigned short *nbrow = s_nbrnode + (f * 24) * NFP + (j - f * NFP);
         // ---- gather the exterior traces (all loads in flight before the first use)
         float ext[TPT][NF];
         int cn[TPT];                                   // packed connectivity of the task's face; INT_MIN = no task
@@ -622,7 +662,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
             cn[i] = c4;
             if (c4 >= 0) {
               const int nb = c4 >> 5;
-              const int nn = __ldg(nbrow + (c4 & 31) * NFP);
+              const int nn = nbrow[(c4 & 31) * NFP];
               const unsigned rel = (unsigned)(nb - k0);
               if (C::INBATCH && rel < (unsigned)nvalid) {    // neighbour inside the batch: its values are in the tile
                 const float *qp = s_q + (rel * NF) * PT + nn;
@@ -698,7 +738,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     const uint16_t *img = P.Bimg + (size_t)hid * C::NSTEP * (C::BSTAGE / 2);
     int slot = 0;
     uint32_t phase = 0;
-    for (int b = worker; b < P.nbatch; b += nworkers) {
+    for (int b = P.bbeg + worker; b < P.nbatch; b += nworkers) {
       for (int st = 0; st < C::NSTEP; ++st) {
         T3_WAIT(emptyB(slot), phase ^ 1, 0);
         if (tc::elect_one()) {
@@ -715,7 +755,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
     const uint64_t descB0 = tc::make_desc(tc::smem_u32(sB), NCH * 16, 128);
     int sa = 0, sb = 0, it = 0;
     uint32_t pa = 0, pb = 0;
-    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+    for (int b = P.bbeg + worker; b < P.nbatch; b += nworkers, ++it) {
       const int set = C::NSETS == 2 ? (it & 1) : 0, use = C::NSETS == 2 ? (it >> 1) : it;
       T3_WAIT(accEmpty(set), (use & 1) ^ 1, 0);
       tc::tc_fence_after();
@@ -746,7 +786,7 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
   } else {
     // =================================================== tile loader: fields, geometric records, connectivity
     int it = 0, uc = 0;
-    for (int b = worker; b < P.nbatch; b += nworkers, ++it) {
+    for (int b = P.bbeg + worker; b < P.nbatch; b += nworkers, ++it) {
       const int k0 = b * EB;
       const int nvalid = min(EB, p.K - k0);
       const int qs = it % NQ, quse = it / NQ;
@@ -762,6 +802,10 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         tc::bulk_g2s(tc::smem_u32(s_geo), p.geo + (size_t)k0 * NGEO, bg, qFull(qs));
         tc::bulk_g2s(tc::smem_u32(s_geo + EB * NGEO * 4), P.conn + (size_t)k0 * 4, bc, qFull(qs));
         if (MODE == MODE_STAGE && p.a != 0.f) tc::prefetch_l2(p.res + (size_t)k0 * NF * PT, bq);
+        if (MODE == MODE_AB3) {
+          tc::prefetch_l2(p.res + (size_t)k0 * NF * PT, bq);
+          tc::prefetch_l2(p.hist2 + (size_t)k0 * NF * PT, bq);
+        }
       }
       __syncwarp();
       if (!TILE) {

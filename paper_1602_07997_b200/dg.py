@@ -35,7 +35,7 @@ class _Options(C.Structure):
 
 
 EXPORTS = ["dg_create", "dg_destroy", "dg_num_fields", "dg_np", "dg_nfp", "dg_num_elements", "dg_node_coords",
-           "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_stage", "dg_ab3_step", "dg_ab3_reset", "dg_last_launch_count",
+           "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_stage", "dg_stage_range", "dg_range_alignment", "dg_element_dt", "dg_ab3_step", "dg_ab3_run", "dg_ab3_reset", "dg_last_launch_count",
            "dg_variant_name", "dg_reference_operators", "dg_geometry", "dg_connectivity", "dg_last_error"]
 
 _lib.dg_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(_Materials), C.POINTER(_Options)]
@@ -53,7 +53,11 @@ _lib.dg_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.dg_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
 _lib.dg_run.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int, C.c_void_p]
 _lib.dg_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
+_lib.dg_stage_range.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int64, C.c_int64, C.c_void_p]
+_lib.dg_range_alignment.argtypes = [C.c_void_p]
+_lib.dg_element_dt.argtypes = [C.c_void_p, C.c_double, C.c_void_p]
 _lib.dg_ab3_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
+_lib.dg_ab3_run.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int, C.c_void_p]
 _lib.dg_ab3_reset.argtypes = [C.c_void_p, C.c_void_p]
 _lib.dg_variant_name.argtypes = [C.c_void_p]
 _lib.dg_variant_name.restype = C.c_char_p
@@ -180,8 +184,25 @@ class Context:
         _check(_lib.dg_stage(self._h, C.c_void_p(d_q_in), C.c_void_p(d_q_out), C.c_float(a), C.c_float(b), C.c_float(dt),
                              C.c_void_p(stream or 0)))
 
+    def stage_range(self, d_q_in: int, d_q_out: int, a: float, b: float, dt: float, k_begin: int, k_end: int,
+                    stream: int | None = None):
+        _check(_lib.dg_stage_range(self._h, C.c_void_p(d_q_in), C.c_void_p(d_q_out), C.c_float(a), C.c_float(b), C.c_float(dt),
+                                   int(k_begin), int(k_end), C.c_void_p(stream or 0)))
+
+    @property
+    def range_alignment(self) -> int:
+        return int(_lib.dg_range_alignment(self._h))
+
+    def element_dt(self, cfl: float = 0.5) -> np.ndarray:
+        out = np.empty(self.K, dtype=np.float64)
+        _check(_lib.dg_element_dt(self._h, float(cfl), _ptr(out)))
+        return out
+
     def ab3_step(self, d_q: int, dt: float, stream: int | None = None):
         _check(_lib.dg_ab3_step(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))
+
+    def ab3_run(self, d_q: int, dt: float, nsteps: int, stream: int | None = None):
+        _check(_lib.dg_ab3_run(self._h, C.c_void_p(d_q), C.c_float(dt), int(nsteps), C.c_void_p(stream or 0)))
 
     def ab3_reset(self, stream: int | None = None):
         _check(_lib.dg_ab3_reset(self._h, C.c_void_p(stream or 0)))

@@ -174,6 +174,11 @@ def random_fields(K: int, model: int, Np: int, seed: int = 3) -> np.ndarray:
 SWEEP_CELLS = {1: 101, 2: 75, 3: 59, 4: 49, 5: 42, 6: 37, 7: 33, 8: 29, 9: 27, 10: 24}
 
 
+# the paper's own problem size (N = 1..8, "approximately 2 M nodes" per mesh): cells per side so that
+# K Np is closest to 2.0e6
+PAPER_CELLS = {1: 44, 2: 32, 3: 26, 4: 21, 5: 18, 6: 16, 7: 14, 8: 13}
+
+
 @dataclass
 class Workload:
     name: str
@@ -244,8 +249,13 @@ def config(i: int, N: int | None = None, model: int | None = None, n: int | None
     elif i == 5:
         w = Workload("C5-elastic-N10-random", ELASTIC, 10, 24, jitter=0.10, materials="random_c5",
                      ic="random", top=BC_FREE, nsteps=20)
+    elif i == 6:                      # not a BASELINE.json config: the paper's size, materials / IC as config 4
+        if N is None or model is None or N not in PAPER_CELLS:
+            raise ValueError("the paper-sized workload needs N in 1..8 and model")
+        w = Workload(f"P-paper-sized-{'acoustic' if model == ACOUSTIC else 'elastic'}-N{N}", model, N,
+                     PAPER_CELLS[N], materials="random", ic="pulse", nsteps=20)
     else:
-        raise ValueError("config index 1..5")
+        raise ValueError("config index 1..6")
     if n is not None:
         w.n = n
         w.name += f"-n{n}"

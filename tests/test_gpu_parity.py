@@ -181,22 +181,40 @@ def test_zero_field_gives_zero_rhs_and_energy_decays(dg):
     assert 0 < e1 < e0
 
 
-def test_ab3_matches_paper_eq4(dg):
-    """The paper's own integrator (eq. (4)): three AB3 steps from zero history."""
+@pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 3, {}), (W.ELASTIC, 5, {"max_ctas": 2}), (W.ELASTIC, 8, {}), (W.ACOUSTIC, 2, {}),
+                                          (W.ELASTIC, 1, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 10, {"max_ctas": 4})])
+def test_ab3_matches_paper_eq4(dg, model, N, opts):
+    """The paper's own integrator (eq. (4)) as a fused epilogue of every stage-kernel family: 24 steps
+    (two start-up steps, reading Q21, then 22 fused AB3 kernels -- with `max_ctas` several batches per persistent
+    CTA; N = 8, 10: padded rows, N = 10: two CTAs per batch) against oracle.timestep.ab3_step; dg_ab3_run in one call, in
+    two calls and step by step give the same bits."""
     from oracle import timestep
-    case = Case(dg, W.config(1, n=2))
+    case = Case(dg, _sweep_case(model, N), **opts)
+    ctx = case.ctx
     q32 = case.initial_fields32()
-    dt = case.dt32(0.2)
+    dt = case.dt32(0.05)
+    stream = torch.cuda.current_stream().cuda_stream
     d_q = torch.from_numpy(q32).cuda()
-    case.ctx.ab3_reset()
-    for _ in range(4):
-        case.ctx.ab3_step(d_q.data_ptr(), dt)
+    ctx.ab3_reset()
+    ctx.ab3_run(d_q.data_ptr(), dt, 24, stream)
     torch.cuda.synchronize()
+    npad = 2 if "pitch=" in ctx.variant_name and f"pitch={ctx.Np}," not in ctx.variant_name else 0
+    assert ctx.last_launch_count == 2 * 6 + 22 + (npad if npad else 0), ctx.last_launch_count      # even number of swaps: no copy back
     q = q32.astype(np.float64)
-    hist = [np.zeros_like(q), np.zeros_like(q)]
-    for _ in range(4):
+    hist = []
+    for _ in range(24):
         timestep.ab3_step(q, hist, dt, case.oracle_rhs)
-    assert rel_l2(d_q.cpu().numpy(), q) <= 1e-5
+    got = d_q.cpu().numpy()
+    assert_close(got, q, 1e-5, f"{ctx.variant_name}: 24 AB3 steps")
+    inc = rel_l2(got.astype(np.float64) - q32, q - q32)
+    assert inc <= 1e-4, (ctx.variant_name, inc)
+    d_b = torch.from_numpy(q32).cuda()
+    ctx.ab3_reset()
+    ctx.ab3_run(d_b.data_ptr(), dt, 7, stream)
+    for _ in range(17):
+        ctx.ab3_step(d_b.data_ptr(), dt, stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_b.cpu().numpy(), got)
 
 
 def test_padded_private_layout_paths(dg):
@@ -217,15 +235,15 @@ def test_padded_private_layout_paths(dg):
     torch.cuda.synchronize()
     assert case.ctx.last_launch_count == 3
     assert np.array_equal(d_q.cpu().numpy(), q32) and np.isfinite(d_r.cpu().numpy()).all()
-    # the paper's AB3 step through the same conversion
-    dta = case.dt32(0.2)
+    # the paper's AB3 step through the same conversion (two start-up steps + three fused AB3 kernels)
+    dta = case.dt32(0.05)
     case.ctx.ab3_reset()
-    for _ in range(3):
+    for _ in range(5):
         case.ctx.ab3_step(d_q.data_ptr(), dta)
     torch.cuda.synchronize()
     q = q32.astype(np.float64)
-    hist = [np.zeros_like(q), np.zeros_like(q)]
-    for _ in range(3):
+    hist = []
+    for _ in range(5):
         timestep.ab3_step(q, hist, dta, case.oracle_rhs)
     assert rel_l2(d_q.cpu().numpy(), q) <= 1e-5
 

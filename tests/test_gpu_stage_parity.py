@@ -227,3 +227,56 @@ def test_element_per_thread_vs_node_per_thread_every_element(dg, model, N):
     assert out[0][0].startswith("simt_elem_per_thread") and out[1][0].startswith("simt_fused")
     err = float((out[0][1] - out[1][1]).double().norm() / out[1][1].double().norm())
     assert err <= 1e-5, (out[0][0], out[1][0], err)
+
+
+# ---------------------------------------------------------------- multi-rate hook: a stage restricted to an element range
+@pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 1, {}), (W.ACOUSTIC, 3, {}), (W.ELASTIC, 3, {}), (W.ELASTIC, 5, {"max_ctas": 2}),
+                                          (W.ELASTIC, 9, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1})])
+def test_stage_range_composes_to_the_full_stage(dg, model, N, opts):
+    """dg_stage_range over [0, k1), [k1, k2), [k2, K) -- the per-level launches of a multi-rate driver
+    -- writes exactly what one dg_stage over the mesh writes, touches nothing outside its range (q_out and the residual),
+    and agrees with the oracle's r_k on the range."""
+    case = Case(dg, _sweep_case(model, N), **opts)
+    ctx = case.ctx
+    al = ctx.range_alignment
+    K = ctx.K
+    k1, k2 = al * max(1, (K // 3) // al), al * max(2, (2 * K // 3) // al)
+    assert 0 < k1 < k2 < K
+    q32 = case.initial_fields32()
+    dt = case.dt32()
+    stream = torch.cuda.current_stream().cuda_stream
+    d_q = torch.from_numpy(q32).cuda()
+    full1, d_full1 = case.gpu_stage(torch, q32, 0.0, B[0], dt)
+    full2, _ = case.gpu_stage(torch, None, A[1], B[1], dt, d_in=d_full1)
+    # the same two stages, range by range
+    d_o1 = torch.full_like(d_q, float("nan"))
+    ctx.stage_range(d_q.data_ptr(), d_o1.data_ptr(), 0.0, B[0], dt, k1, k2, stream)
+    torch.cuda.synchronize()
+    part = d_o1.cpu().numpy()
+    assert np.isnan(part[:k1]).all() and np.isnan(part[k2:]).all(), "dg_stage_range wrote outside its range"
+    assert np.array_equal(part[k1:k2], full1[k1:k2])
+    want = q32[k1:k2].astype(np.float64) + np.float32(B[0]) * np.float64(dt) * case.oracle_rhs(q32.astype(np.float64), np.arange(k1, k2))
+    assert_close(part[k1:k2], want, RHS_TOL, f"{ctx.variant_name}: stage on elements [{k1}, {k2})")
+    for lo, hi in ((0, k1), (k2, K)):
+        ctx.stage_range(d_q.data_ptr(), d_o1.data_ptr(), 0.0, B[0], dt, lo, hi, stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_o1.cpu().numpy(), full1)
+    d_o2 = torch.full_like(d_q, float("nan"))
+    for lo, hi in ((k2, K), (0, k1), (k1, k2)):                 # any order: ranges are independent within a stage
+        ctx.stage_range(d_o1.data_ptr(), d_o2.data_ptr(), A[1], B[1], dt, lo, hi, stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_o2.cpu().numpy(), full2), "residual carried differently range by range"
+    ctx.stage_range(d_q.data_ptr(), d_o1.data_ptr(), 0.0, B[0], dt, k1, k1, stream)     # empty range: no-op
+    assert ctx.last_launch_count == 0
+    with pytest.raises(dg.DGError):
+        ctx.stage_range(d_q.data_ptr(), d_o1.data_ptr(), 0.0, B[0], dt, k1 + (1 if al > 1 else K + 1), k2, stream)
+    with pytest.raises(dg.DGError):
+        ctx.stage_range(d_q.data_ptr(), d_q.data_ptr(), 0.0, B[0], dt, 0, K, stream)
+
+
+def test_stage_range_is_refused_on_padded_rows(dg):
+    case = Case(dg, _sweep_case(W.ELASTIC, 4), variant=4)
+    d = torch.zeros(case.ctx.shape, dtype=torch.float32, device="cuda")
+    o = torch.zeros_like(d)
+    with pytest.raises(dg.DGError):
+        case.ctx.stage_range(d.data_ptr(), o.data_ptr(), 0.0, 1.0, 1e-3, 0, case.ctx.K)

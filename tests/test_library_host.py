@@ -166,3 +166,22 @@ def test_boundary_tags_follow_the_callers_face_numbering(dg, refelems):
             assert not np.all(lt[(lt > 0) & (bad.geometry()["nrm"][..., 2] > 0.99)] == W.BC_FREE)
         except dg.DGError as e:                      # or the swap leaves a boundary face untagged: also a loud failure
             assert e.code == -2
+
+
+def test_element_dt_levels_for_multirate(dg, refelems):
+    """dg_element_dt (multi-rate hook): every element's own stable step by the rule of DESIGN.md Q10; the
+    global step of dg_stable_dt is its minimum; on a mesh with one refined corner the steps spread over > 2 octaves,
+    which is what a local time stepping driver bins into levels."""
+    vxyz, etov, _ = W.kuhn_cube(3, 0.05, seed=1)
+    vxyz = vxyz ** 2.5                                   # grade the mesh towards the origin (walls stay planar)
+    K = etov.shape[0]
+    rho, vp, vs = W.random_elastic_materials(K, seed=2)
+    ctx = dg.Context(vxyz, etov, 4, dg.ELASTIC, rho, vp, vs, None, device=-1)
+    m = omesh.build(refelems(4), vxyz, etov, None)
+    want = 0.5 / (25.0 * vp * m.Fscale.max(axis=1))
+    got = ctx.element_dt(0.5)
+    assert np.abs(got / want - 1).max() < 1e-12
+    assert abs(got.min() / ctx.stable_dt(0.5) - 1) < 1e-12
+    levels = np.floor(np.log2(got / got.min())).astype(int)
+    assert levels.max() >= 2 and (np.bincount(levels) > 0).sum() >= 3
+    assert ctx.range_alignment in (1, 14, 32) or ctx.range_alignment > 0

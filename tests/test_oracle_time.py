@@ -100,6 +100,33 @@ def test_lsrk_temporal_order_vs_matrix_exponential_T12(refelems, model):
     assert np.linalg.norm(q1 - tay) < 50 * np.linalg.norm(dt ** 5 * np.linalg.matrix_power(A, 5) @ q0.ravel())
 
 
+def test_ab3_with_lsrk_startup_is_third_order(refelems):
+    """eq. (4) with the start-up of DESIGN.md reading Q21 against the matrix exponential: halving dt
+    divides the error by 8; started from a zero history instead (no start-up) the same scheme is first order."""
+    ref, m, shape, rhs, cmax = _small_system(refelems, "acoustic", 2)
+    n = int(np.prod(shape))
+    A = np.empty((n, n))
+    for j in range(n):
+        e = np.zeros(n); e[j] = 1.0
+        A[:, j] = rhs(e.reshape(shape)).ravel()
+    q0 = np.random.default_rng(4).standard_normal(shape)
+    T = 0.05
+    exact = (scipy.linalg.expm(A * T) @ q0.ravel()).reshape(shape)
+    errs, errs0 = [], []
+    for steps in (40, 80, 160):
+        q, hist = q0.copy(), []
+        for _ in range(steps):
+            timestep.ab3_step(q, hist, T / steps, rhs)
+        errs.append(np.linalg.norm(q - exact) / np.linalg.norm(exact))
+        q, hist = q0.copy(), [np.zeros(shape), np.zeros(shape)]
+        for _ in range(steps):
+            timestep.ab3_step(q, hist, T / steps, rhs)
+        errs0.append(np.linalg.norm(q - exact) / np.linalg.norm(exact))
+    assert errs[0] < 1e-2
+    assert 6.5 < errs[0] / errs[1] < 9.5 and 6.5 < errs[1] / errs[2] < 9.5           # third order
+    assert 1.6 < errs0[0] / errs0[1] < 2.4 and errs0[2] > 20 * errs[2]                # zero history: first order
+
+
 # ---------------------------------------------------------------- T10/T11 acoustic standing mode
 def _mass_norm(ref, m, e):
     return np.sqrt(sum(np.sum(m.J * np.einsum("kn,nm,km->k", e[:, f], ref.M, e[:, f])) for f in range(e.shape[1])))
