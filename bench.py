@@ -380,6 +380,8 @@ def run_ours(a):
         opts["groups_per_cta"] = a.G
     if a.variant:
         opts["variant"] = a.variant
+    if a.surface == "interface":
+        opts["surface"] = 1
     ctx = dg.from_workload(w, device=local, **opts)
     xyz = ctx.node_coords()
     q0 = w.initial_fields(xyz).astype(np.float32)
@@ -468,7 +470,7 @@ def run_ours(a):
     del d_q, h_out
     torch.cuda.empty_cache()
     if rank == 0:
-        if world == 1 and not a.no_sweep and not ab3 and a.config == 2 and not a.variant:
+        if world == 1 and not a.no_sweep and not ab3 and a.config == 2 and not a.variant and a.surface == "element":
             log = (lambda r: print("sweep " + json.dumps(r), file=sys.stderr, flush=True))
             roof["sweep_columns"] = SWEEP_COLUMNS
             roof["sweep"] = sweep_rows(torch, dg, local, sampler, steps=a.sweep_steps, repeats=a.repeats, log=log)
@@ -525,6 +527,8 @@ def main():
     ap.add_argument("--E", type=int, default=0)
     ap.add_argument("--G", type=int, default=0)
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 fused FP32 SIMT kernel, 4 pipelined tcgen05 BF16x3 kernel")
+    ap.add_argument("--surface", default="element", choices=["element", "interface"],
+                    help="interface: the paper's interface-centric surface kernel feeds the stage kernel (dg_options.surface = 1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 degree sweep of the default run")
     ap.add_argument("--sweep-steps", type=int, default=5)

@@ -88,6 +88,15 @@ typedef struct {
   int max_ctas;               /* 0 = auto (one persistent CTA per SM); > 0 caps the grid of the
                                  tensor-core variant so that small test meshes give every CTA
                                  several batches (tests); < 0: DG_ERR_ARG                         */
+  int surface;                /* 0 = element-centric (default): the stage kernel gathers the exterior traces and evaluates
+                                 the penalty terms of its own elements; 1 = interface-centric (the surface kernel of the
+                                 paper's SGEMM strategy): a separate kernel visits every interface once, one
+                                 thread per face node computes the terms of both sides into a face buffer
+                                 [K][Nfields][4 Nfp], and the stage kernel lifts from it (one more launch per evaluation) */
+  int64_t owned_elements;     /* 0 = all; > 0: the first `owned_elements` elements of the mesh are this process's own, the
+                                 rest are ghost copies of other processes' elements (dg_partition_*): every device entry
+                                 point advances / evaluates the owned elements only; ghosts are read through the
+                                 connectivity and filled by dg_halo_unpack                                          */
 } dg_options;
 
 /* Build a context: reference operators for degree N (1..10), geometric factors, connectivity,
@@ -157,6 +166,29 @@ int dg_reference_operators(const dg_ctx *ctx, double *Dr, double *Ds, double *Dt
  * node: elemP, nodeP [K][4Nfp] (boundary faces: the element's own node), bctag [K][4].           */
 int dg_geometry(const dg_ctx *ctx, double *G, double *J, double *nrm, double *fscale);
 int dg_connectivity(const dg_ctx *ctx, int32_t *elemP, int32_t *nodeP, int8_t *bctag);
+
+/* ---- multi-GPU: element partition and halo exchange (one process per GPU) ------------------
+ * The element list is cut into `nranks` contiguous slabs.  dg_partition_create builds, for one rank, its local mesh =
+ * its own elements followed by ghost copies of the elements across its cut faces (vertex numbers stay global: pass the
+ * same vxyz to dg_create, with dg_options.owned_elements = dg_partition_num_owned), and per peer rank the lists of faces
+ * (4 * local element + face, the library's face numbering) whose face-node values are sent (own elements) and received
+ * (ghosts), in matching order on both sides.  Host only.  Before every stage:
+ *   dg_halo_pack(send faces) -> exchange the buffers [nfaces][Nfields][Nfp] float (NCCL send/recv or peer copies; the
+ *   caller's plumbing) -> dg_halo_unpack(recv faces) -> dg_stage.  Only face traces move: Nfields Nfp floats per cut face
+ *   and direction.  d_faces are DEVICE copies of the lists; d_q is in the caller's layout [K][Nfields][Np].            */
+typedef struct dg_part dg_part;
+int dg_partition_create(dg_part **out, const dg_mesh *mesh, int nranks, int rank);
+int dg_partition_destroy(dg_part *part);
+int64_t dg_partition_num_owned(const dg_part *part);
+int64_t dg_partition_num_ghost(const dg_part *part);
+int dg_partition_global_ids(const dg_part *part, int64_t *ids /* [owned + ghost] */);
+int dg_partition_local_mesh(const dg_part *part, int32_t *etov /* [owned + ghost][4] */, int8_t *bc /* [owned + ghost][4] */);
+int dg_partition_num_peers(const dg_part *part);
+int dg_partition_peer(const dg_part *part, int i, int *rank, int64_t *nsend, int64_t *nrecv);
+int dg_partition_halo_faces(const dg_part *part, int i, int32_t *send_faces /* [nsend] */, int32_t *recv_faces /* [nrecv] */);
+int dg_halo_pack(dg_ctx *ctx, const float *d_q, const int32_t *d_faces, int64_t nfaces, float *d_buf, void *cuda_stream);
+int dg_halo_unpack(dg_ctx *ctx, float *d_q, const int32_t *d_faces, int64_t nfaces, const float *d_buf, void *cuda_stream);
+int64_t dg_num_owned_elements(const dg_ctx *ctx);
 
 const char *dg_last_error(void);
 

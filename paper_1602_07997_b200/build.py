@@ -58,7 +58,7 @@ def build(force: bool = False, jobs: int | None = None, verbose: bool = False) -
             src = os.path.join(CSRC, "stage_inst.cu")
             if force or not _newer(o, [src] + hdrs):
                 tasks.append([nvcc, *ARCH, *flags, f"-DDG_MODEL={model}", f"-DDG_N={N}", "-c", src, "-o", o])
-    for name in ("dg_api.cu", "host_setup.cpp"):
+    for name in ("dg_api.cu", "host_setup.cpp", "partition.cpp"):
         src = os.path.join(CSRC, name)
         o = os.path.join(OBJ, name.rsplit(".", 1)[0] + ".o")
         objs.append(o)

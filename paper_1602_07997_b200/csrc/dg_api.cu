@@ -17,6 +17,7 @@
 #include "host_setup.hpp"
 #include "kernels.cuh"
 #include "tc3_kernels.cuh"
+#include "iface_kernels.cuh"
 
 // per-(model, degree) kernel getters from stage_inst.cu
 #define DG_DECL(m, n)                                              \
@@ -25,6 +26,7 @@
   extern "C" const void *dgk_get_tc3_kernel_##m##_##n(int);       \
   extern "C" const void *dgk_get_epk_kernel_##m##_##n(int);       \
   extern "C" int dgk_epk_upload_##m##_##n(const float *, const float *, const unsigned short *, const int *); \
+  extern "C" const void *dgk_get_iface_kernel_##m##_##n(void);   \
   extern "C" int dgk_tc3_info_##m##_##n(int);
 #define DG_DECL_ALL(m) \
   DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
@@ -53,12 +55,19 @@ const tc_getter EPK_KERNELS[2][11] = {DG_ROW(0, dgk_get_epk_kernel_), DG_ROW(1, 
 const epk_upload_fn EPK_UPLOAD[2][11] = {DG_ROW(0, dgk_epk_upload_), DG_ROW(1, dgk_epk_upload_)};
 const tc_getter TC3_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc3_kernel_), DG_ROW(1, dgk_get_tc3_kernel_)};
 const info_getter TC3_INFO[2][11] = {DG_ROW(0, dgk_tc3_info_), DG_ROW(1, dgk_tc3_info_)};
+typedef const void *(*iface_getter)(void);
+const iface_getter IFACE_KERNELS[2][11] = {DG_ROW(0, dgk_get_iface_kernel_), DG_ROW(1, dgk_get_iface_kernel_)};
 
 thread_local std::string g_err;
 int fail(int code, const std::string &msg) {
   g_err = msg;
   return code;
 }
+}  // namespace
+namespace dgapi {
+int fail(int code, const std::string &msg) { return ::fail(code, msg); }
+}  // namespace dgapi
+namespace {
 #define CUDA_TRY(x)                                                                                   \
   do {                                                                                                \
     cudaError_t e_ = (x);                                                                             \
@@ -83,11 +92,28 @@ __global__ void repitch_kernel(float *__restrict__ dst, int dpitch, const float 
   }
 }
 
+// halo exchange (partition.cpp): face-node values of all fields of the listed faces (4 element + face) <-> a dense buffer
+// [face][field][face node]; the same routine on the sending side (pack, owned elements) and the receiving side (unpack, ghosts)
+template <bool PACK>
+__global__ void halo_kernel(float *__restrict__ q, float *__restrict__ buf, const int *__restrict__ faces, const unsigned short *__restrict__ fmask,
+                            int nf, int np, int nfp, size_t n) {
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+    const size_t ent = t / (unsigned)(nf * nfp);
+    const int rem = (int)(t - ent * (unsigned)(nf * nfp));
+    const int c = rem / nfp, i = rem - c * nfp;
+    const int fa = faces[ent];
+    float *qq = q + ((size_t)(fa >> 2) * nf + c) * np + fmask[(fa & 3) * nfp + i];
+    if (PACK) buf[t] = *qq;
+    else *qq = buf[t];
+  }
+}
+
 }  // namespace dgk
 
 struct dg_ctx {
   int N = 0, Np = 0, Nfp = 0, model = 0, NF = 0, device = -1;
   int64_t K = 0;
+  int64_t K_active = 0;                          // elements the stage kernels advance (dg_options.owned_elements; the rest are ghosts)
   dgh::RefElem ref;
   dgh::HostMesh mesh;
   std::vector<double> cmax;
@@ -109,6 +135,14 @@ struct dg_ctx {
   struct TmapEntry { std::array<CUtensorMap, 5> m; bool pinned; uint64_t stamp; };
   std::map<const void *, TmapEntry> tmaps;
   uint64_t tmap_clock = 0;
+  // interface-centric surface step (dg_options.surface = 1, iface_kernels.cuh)
+  int surface = 0;
+  const void *k_iface = nullptr;
+  float *d_pflux = nullptr;                      // [K][Nf][4 Nfp] penalty terms times g^sur
+  int *d_ifaces = nullptr;                       // interior owner faces, then boundary faces
+  unsigned short *d_nbrface = nullptr;
+  int n_int = 0, n_bnd = 0;
+  int iface_launches = 0;                        // interface kernels launched by the current API call
   int max_ctas = 0;                              // dg_options.max_ctas: cap on the persistent grid (tests; 0 = one CTA per SM)
   float *d_res = nullptr, *d_q2 = nullptr, *d_hist[3] = {nullptr, nullptr, nullptr};
   int hist_head = 0;                             // d_hist[hist_head] = r^{m-1}, d_hist[(hist_head + 1) % 3] = r^{m-2}
@@ -151,6 +185,7 @@ void free_device(dg_ctx *c) {
   cudaFree(c->d_DT); cudaFree(c->d_LT); cudaFree(c->d_Bimg); cudaFree(c->d_conn); cudaFree(c->d_qa); cudaFree(c->d_geo); cudaFree(c->d_nbr); cudaFree(c->d_fcode);
   cudaFree(c->d_fmask); cudaFree(c->d_nbrnode); cudaFree(c->d_res); cudaFree(c->d_q2);
   for (float *&h : c->d_hist) cudaFree(h);
+  cudaFree(c->d_pflux); cudaFree(c->d_ifaces); cudaFree(c->d_nbrface);
 }
 
 void build_geo_records(const dg_ctx *c, const dg_materials *mat, std::vector<float> &geo) {
@@ -257,7 +292,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     c->k_ab3 = TC3_KERNELS[c->model][c->N](dgk::MODE_AB3);
     const info_getter info = TC3_INFO[c->model][c->N];
     const int EB = info(1);
-    c->nbatch = (int)((c->K + EB - 1) / EB);
+    c->nbatch = (int)((c->K_active + EB - 1) / EB);
     c->NT = dgk::T3_THREADS;
     c->smem = (size_t)info(0);
     c->epi_cw = info(9);
@@ -278,7 +313,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
     c->k_ab3 = EPK_KERNELS[c->model][c->N](dgk::MODE_AB3);
     c->NT = 128;
     c->smem = 0;
-    c->grid = (int)((c->K + 127) / 128);
+    c->grid = (int)((c->K_active + 127) / 128);
     char buf[128];
     snprintf(buf, sizeof buf, "simt_elem_per_thread<%s,N=%d,threads=128,operators in constant memory>", c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N);
     c->variant = buf;
@@ -304,7 +339,7 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
   if (c->NT > 1024) throw std::invalid_argument("groups_per_cta too large: more than 1024 threads");
   c->smem = SMEM[c->model][c->N](G * E);
   if (c->smem > 227 * 1024) throw std::invalid_argument("batch does not fit in shared memory");
-  c->grid = (int)((c->K + (int64_t)G * E - 1) / ((int64_t)G * E));
+  c->grid = (int)((c->K_active + (int64_t)G * E - 1) / ((int64_t)G * E));
   char buf[128];
   snprintf(buf, sizeof buf, "simt_fused<%s,N=%d,E=%d,G=%d,threads=%d,smem=%zu>", c->model == DG_ACOUSTIC ? "acoustic" : "elastic",
            c->N, E, G, c->NT, c->smem);
@@ -345,7 +380,7 @@ std::array<CUtensorMap, 5> tensor_maps(dg_ctx *c, const void *ptr, bool pin = fa
   // (no-tile configurations); [3], [4]: the AB3 epilogue's boxes of epi_cw / 2 nodes.  Swizzle = the box's row length
   for (int h = 0; h < 5; ++h) {
     const int width = h == 2 ? 16 : (h < 2 ? c->epi_cw : c->epi_cw / 2);
-    const cuuint64_t dims[2] = {(cuuint64_t)c->PT, (cuuint64_t)c->K * c->NF};
+    const cuuint64_t dims[2] = {(cuuint64_t)c->PT, (cuuint64_t)c->K_active * c->NF};   // (ghost rows are never loaded or stored by boxes)
     const cuuint64_t strides[1] = {(cuuint64_t)c->PT * 4};
     const int height = h == 2 ? 128 : ((h == 0 || h == 3) ? 32 : rlast);
     const cuuint32_t box[2] = {(cuuint32_t)width, (cuuint32_t)height};
@@ -370,15 +405,28 @@ int range_alignment(const dg_ctx *c) {
 // AB3 launches (kernel == c->k_ab3): hist1 = r^{m-1}, hist2 = r^{m-2} (inputs), rhs = the buffer that receives r^m
 int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out, float *rhs, float a, float b, float dt,
                  cudaStream_t st, int64_t kbeg = 0, int64_t kend = -1, float *hist1 = nullptr, const float *hist2 = nullptr) {
-  if (kend < 0) kend = c->K;
+  if (kend < 0) kend = c->K_active;
   if (kbeg >= kend) return DG_OK;
   dgk::StageParams p;
   p.q_in = q_in; p.q_out = q_out; p.res = hist1 ? hist1 : c->d_res; p.rhs = rhs; p.hist2 = hist2;
   p.DT = c->d_DT; p.LT = c->d_LT; p.geo = c->d_geo; p.nbr = c->d_nbr; p.fcode = c->d_fcode;
   p.fmask = c->d_fmask; p.nbrnode = c->d_nbrnode;
   p.K = (int)kend; p.kbeg = (int)kbeg; p.G = c->G; p.a = a; p.b = b; p.dt = dt;
+  p.pflux = nullptr;
+  if (c->surface) {                              // rows a4 + a5 by interfaces, into the face buffer the stage kernel lifts from
+    dgk::IfaceParams ip;
+    ip.q = q_in; ip.pflux = c->d_pflux; ip.geo = c->d_geo; ip.nbr = c->d_nbr; ip.fcode = c->d_fcode; ip.faces = c->d_ifaces;
+    ip.fmask = c->d_fmask; ip.nbrnode = c->d_nbrnode; ip.nbrface = c->d_nbrface;
+    ip.nint = c->n_int; ip.nbnd = c->n_bnd; ip.pitch = c->tc3 ? c->PT : c->Np;
+    const long long nthreads = (long long)(c->n_int + c->n_bnd) * c->Nfp;
+    void *iargs[] = {&ip};
+    cudaError_t e = cudaLaunchKernel(c->k_iface, dim3((unsigned)((nthreads + 255) / 256)), dim3(256), iargs, 0, st);
+    if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " launching the interface kernel");
+    p.pflux = c->d_pflux;
+    ++c->iface_launches;
+  }
   int grid = c->grid;
-  if (kbeg != 0 || kend != c->K) {
+  if (kbeg != 0 || kend != c->K_active) {
     const int unit = c->epk ? 128 : range_alignment(c);
     grid = (int)((kend - kbeg + unit - 1) / unit);
   }
@@ -389,7 +437,7 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   if (c->tc3) {
     if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
     tp3.s = p;
-    tp3.s.K = (int)c->K;                          // (the kernel bounds a ragged last batch by the mesh, ranges by batches)
+    tp3.s.K = (int)c->K_active;                   // (the kernel bounds a ragged last batch by the advanced elements, ranges by batches)
     tp3.Bimg = c->d_Bimg;
     tp3.conn = c->d_conn;
     const int EB = range_alignment(c), nsplit = TC3_INFO[c->model][c->N](4);
@@ -430,7 +478,8 @@ int check_device_ctx(const dg_ctx *c) {
 #define DG_ENTER_DEVICE(c)                                \
   if (int e_ = check_device_ctx(c)) return e_;            \
   DeviceGuard guard_((c)->device);                        \
-  if (!guard_.ok) return fail(DG_ERR_CUDA, "cuda: cannot select the context's device")
+  if (!guard_.ok) return fail(DG_ERR_CUDA, "cuda: cannot select the context's device");   \
+  (c)->iface_launches = 0
 
 }  // namespace
 
@@ -457,6 +506,10 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
     c->K = mesh->K;
     c->device = opts ? opts->device : 0;
     c->max_ctas = opts ? opts->max_ctas : 0;
+    c->K_active = (opts && opts->owned_elements > 0) ? opts->owned_elements : c->K;
+    if (c->K_active > c->K) throw std::invalid_argument("owned_elements exceeds the number of elements");
+    c->surface = opts ? opts->surface : 0;
+    if (c->surface != 0 && c->surface != 1) throw std::invalid_argument("surface must be 0 (element-centric) or 1 (interface-centric)");
     if (c->max_ctas < 0) throw std::invalid_argument("max_ctas must be >= 0");
     for (int64_t k = 0; k < c->K; ++k) {
       const double rho = mat->rho[k], cp = mat->c_or_vp[k];
@@ -546,6 +599,25 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         CUDA_TRY(cudaMemset(h, 0, nqp * sizeof(float)));
       }
       CUDA_TRY(cudaMemset(c->d_res, 0, nqp * sizeof(float)));
+      if (c->surface) {
+        // one entry per interface (listed by the side with the smaller element number), boundary faces behind
+        std::vector<int> faces, bnd;
+        for (int64_t k = 0; k < c->K; ++k)
+          for (int f = 0; f < 4; ++f) {
+            const int32_t nb = c->mesh.nbr[4 * k + f];
+            if (nb < 0) bnd.push_back((int)(4 * k + f));
+            else if (nb > k) faces.push_back((int)(4 * k + f));
+          }
+        c->n_int = (int)faces.size();
+        c->n_bnd = (int)bnd.size();
+        faces.insert(faces.end(), bnd.begin(), bnd.end());
+        c->d_ifaces = upload(faces);
+        std::vector<unsigned short> nbrface(c->ref.nbrface.begin(), c->ref.nbrface.end());
+        c->d_nbrface = upload(nbrface);
+        CUDA_TRY(cudaMalloc(&c->d_pflux, (size_t)c->K * c->NF * 4 * Nfp * sizeof(float)));
+        c->k_iface = IFACE_KERNELS[c->model][c->N]();
+        c->variant += " + interface-centric surface kernel";
+      }
       if (c->tc3) {                              // descriptors of the library's own buffers: encoded once, never evicted
         tensor_maps(c, c->d_res, true);
         tensor_maps(c, c->d_q2, true);
@@ -691,7 +763,9 @@ int dg_rhs(dg_ctx *c, const float *d_q, float *d_rhs, void *stream) {
   if (!d_q || !d_rhs) return fail(DG_ERR_ARG, "NULL device pointer");
   if (d_q == d_rhs) return fail(DG_ERR_ARG, "dg_rhs: d_q and d_rhs must differ");
   c->last_launches = 0;
-  return eval_rhs(c, d_q, d_rhs, (cudaStream_t)stream, c->last_launches);
+  const int rc = eval_rhs(c, d_q, d_rhs, (cudaStream_t)stream, c->last_launches);
+  c->last_launches += c->iface_launches;
+  return rc;
 }
 
 int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
@@ -712,7 +786,7 @@ int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
       if (int e = copy_rows(c, d_q, c->Np, cur, c->PT, st)) return e;
       launches = 5 * nsteps + 2;
     }
-    c->last_launches = launches;
+    c->last_launches = launches + c->iface_launches;
     return DG_OK;
   }
   float *cur = d_q, *oth = c->d_q2;
@@ -727,7 +801,7 @@ int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
     if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e));
     ++launches;
   }
-  c->last_launches = launches;
+  c->last_launches = launches + c->iface_launches;
   return DG_OK;
 }
 
@@ -739,14 +813,39 @@ int dg_stage(dg_ctx *c, const float *d_q_in, float *d_q_out, float a, float b, f
   if (d_q_in == d_q_out) return fail(DG_ERR_ARG, "dg_stage: d_q_in and d_q_out must differ (neighbours read the stage input)");
   cudaStream_t st = (cudaStream_t)stream;
   if (!padded(c)) {
-    c->last_launches = 1;
+    c->last_launches = 1 + c->surface;
     return launch_stage(c, c->k_stage, d_q_in, d_q_out, nullptr, a, b, dt, st);
   }
   if (int e = copy_rows(c, c->d_qa, c->PT, d_q_in, c->Np, st)) return e;
   if (int e = launch_stage(c, c->k_stage, c->d_qa, c->d_q2, nullptr, a, b, dt, st)) return e;
-  c->last_launches = 3;
+  c->last_launches = 3 + c->surface;
   return copy_rows(c, d_q_out, c->Np, c->d_q2, c->PT, st);
 }
+
+static int halo_move(dg_ctx *c, float *d_q, const int32_t *d_faces, int64_t nfaces, float *d_buf, void *stream, bool pack) {
+  if (!d_q || !d_buf || !d_faces || nfaces < 0) return fail(DG_ERR_ARG, "bad argument");
+  c->last_launches = 0;
+  if (nfaces == 0) return DG_OK;
+  const size_t n = (size_t)nfaces * c->NF * c->Nfp;
+  const int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 16);
+  if (pack) dgk::halo_kernel<true><<<blocks, 256, 0, (cudaStream_t)stream>>>(d_q, d_buf, d_faces, c->d_fmask, c->NF, c->Np, c->Nfp, n);
+  else dgk::halo_kernel<false><<<blocks, 256, 0, (cudaStream_t)stream>>>(d_q, d_buf, d_faces, c->d_fmask, c->NF, c->Np, c->Nfp, n);
+  if (cudaGetLastError() != cudaSuccess) return fail(DG_ERR_CUDA, "cuda: halo kernel launch failed");
+  c->last_launches = 1;
+  return DG_OK;
+}
+
+int dg_halo_pack(dg_ctx *c, const float *d_q, const int32_t *d_faces, int64_t nfaces, float *d_buf, void *stream) {
+  DG_ENTER_DEVICE(c);
+  return halo_move(c, const_cast<float *>(d_q), d_faces, nfaces, d_buf, stream, true);
+}
+
+int dg_halo_unpack(dg_ctx *c, float *d_q, const int32_t *d_faces, int64_t nfaces, const float *d_buf, void *stream) {
+  DG_ENTER_DEVICE(c);
+  return halo_move(c, d_q, d_faces, nfaces, const_cast<float *>(d_buf), stream, false);
+}
+
+int64_t dg_num_owned_elements(const dg_ctx *c) { return c ? c->K_active : (int64_t)fail(DG_ERR_ARG, "NULL context"); }
 
 int dg_range_alignment(const dg_ctx *c) { return c ? range_alignment(c) : fail(DG_ERR_ARG, "NULL context"); }
 
@@ -755,11 +854,11 @@ int dg_stage_range(dg_ctx *c, const float *d_q_in, float *d_q_out, float a, floa
   DG_ENTER_DEVICE(c);
   if (!d_q_in || !d_q_out) return fail(DG_ERR_ARG, "NULL device pointer");
   if (d_q_in == d_q_out) return fail(DG_ERR_ARG, "dg_stage_range: d_q_in and d_q_out must differ");
-  if (k_begin < 0 || k_end > c->K || k_begin > k_end) return fail(DG_ERR_ARG, "dg_stage_range: need 0 <= k_begin <= k_end <= K");
-  if (k_begin % range_alignment(c) != 0 || (k_end % range_alignment(c) != 0 && k_end != c->K))
+  if (k_begin < 0 || k_end > c->K_active || k_begin > k_end) return fail(DG_ERR_ARG, "dg_stage_range: need 0 <= k_begin <= k_end <= K (owned elements)");
+  if (k_begin % range_alignment(c) != 0 || (k_end % range_alignment(c) != 0 && k_end != c->K_active))
     return fail(DG_ERR_ARG, "dg_stage_range: k_begin and k_end must be multiples of dg_range_alignment() (k_end may be K)");
   if (padded(c)) return fail(DG_ERR_ARG, "dg_stage_range: not available for degrees whose rows the library pads (N = 2, 4, 8, 10 on the tensor-core variant); create the context with variant = 1");
-  c->last_launches = k_begin < k_end ? 1 : 0;
+  c->last_launches = k_begin < k_end ? 1 + c->surface : 0;
   return launch_stage(c, c->k_stage, d_q_in, d_q_out, nullptr, a, b, dt, (cudaStream_t)stream, k_begin, k_end);
 }
 
@@ -823,7 +922,7 @@ int dg_ab3_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
     if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e));
     ++launches;
   }
-  c->last_launches = launches;
+  c->last_launches = launches + c->iface_launches;
   return DG_OK;
 }
 

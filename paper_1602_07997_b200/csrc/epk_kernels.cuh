@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
     // (a third of the gather instructions; the kernel is bound by the L1/LSU pipe, the ALUs are idle)
     constexpr bool VGATHER = NP == 4 && MODEL == 0;              // (elastic N = 1: nine vectors per face cost more registers than they save)
     float4 nq[VGATHER ? NF : 1];
-    if (VGATHER && nb >= 0) {
+    if (VGATHER && nb >= 0 && !p.pflux) {
       const float4 *src = reinterpret_cast<const float4 *>(p.q_in + (size_t)nb * NV);
 #pragma unroll
       for (int c = 0; c < NF; ++c) nq[c] = __ldg(src + c);
@@ -191,7 +191,10 @@ __global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
       float um[NF], F[NF];
 #pragma unroll
       for (int c = 0; c < NF; ++c) um[c] = q[c * NP + nm];
-      if (MODEL == 0) {
+      if (p.pflux) {                                                   // interface-centric surface step: terms from the face buffer
+#pragma unroll
+        for (int c = 0; c < NF; ++c) F[c] = __ldg(p.pflux + ((size_t)k * NF + c) * NFACE + j);
+      } else if (MODEL == 0) {
         float dp, dvn;
         if (nb >= 0) {
           const int nn = c_epk_nbrnode[(f * 24 + code) * NFP + i];

@@ -305,6 +305,7 @@ void build_refelem(int N, RefElem &ref) {
   }
   // ---- exterior-trace node table by barycentric matching on the reference faces
   ref.nbrnode.assign((size_t)4 * 4 * 6 * Nfp, 0xFFFF);
+  ref.nbrface.assign((size_t)4 * 4 * 6 * Nfp, 0xFFFF);
   auto bary = [&](int n, int v) {
     switch (v) {
       case 0: return -(1.0 + ref.r[n] + ref.s[n] + ref.t[n]) / 2.0;
@@ -318,7 +319,7 @@ void build_refelem(int N, RefElem &ref) {
       for (int s = 0; s < 6; ++s)
         for (int i = 0; i < Nfp; ++i) {
           const int n = ref.fmask[f * Nfp + i];
-          int found = -1;
+          int found = -1, found_ii = -1;
           for (int ii = 0; ii < Nfp; ++ii) {
             const int nn = ref.fmask[g * Nfp + ii];
             bool ok = true;
@@ -327,10 +328,12 @@ void build_refelem(int N, RefElem &ref) {
             if (ok) {
               if (found >= 0) throw std::runtime_error("reference element: ambiguous face-node match");
               found = nn;
+              found_ii = ii;
             }
           }
           if (found < 0) throw std::runtime_error("reference element: face node sets are not symmetric");
           ref.nbrnode[(((size_t)f * 4 + g) * 6 + s) * Nfp + i] = (uint16_t)found;
+          ref.nbrface[(((size_t)f * 4 + g) * 6 + s) * Nfp + i] = (uint16_t)found_ii;
         }
 }
 

@@ -18,6 +18,7 @@ struct RefElem {
   // exterior-trace node table: for my face f, neighbour face g, vertex correspondence s (0..5):
   // nbrnode[((f*4+g)*6+s)*Nfp + i] = volume node (in the neighbour) that coincides with my face node i
   std::vector<uint16_t> nbrnode;
+  std::vector<uint16_t> nbrface;        // same indexing: that node's position i' on the neighbour's face g (fmask[g][i'] = nbrnode[...])
 };
 
 // the six correspondences: neighbour face-local vertex PERMS[s][j] coincides with my face-local vertex j

@@ -27,6 +27,8 @@ struct StageParams {
   float *__restrict__ res;
   float *__restrict__ rhs;
   const float *__restrict__ hist2;           // MODE_AB3: r^{m-2}
+  const float *__restrict__ pflux;           // interface-centric surface step (iface_kernels.cuh): [K][Nf][4 Nfp] penalty terms
+                                             // times g^sur, computed beforehand; NULL = gather and evaluate them here
   const float *__restrict__ DT;              // [3][Np][Np]  DT[d][m][n] = D_d[n][m]
   const float *__restrict__ LT;              // [4Nfp][Np]   LT[j][n]    = LIFT[n][j]
   const float *__restrict__ geo;             // [K][GEO_*]
@@ -135,6 +137,21 @@ __global__ void stage_kernel(const StageParams p) {
     const int e = it / NFACE, j = it - e * NFACE;
     const int f = j / NFP, i = j - f * NFP;
     const float *g = s_geo + e * NGEO;
+    if (p.pflux) {                              // penalty terms from the face buffer
+      const float *src = p.pflux + ((size_t)(k0 + e) * NF) * NFACE + j;
+      const bool ok = e < nvalid;
+      float F[NF];
+#pragma unroll
+      for (int c = 0; c < NF; ++c) F[c] = ok ? __ldg(src + (size_t)c * NFACE) : 0.f;
+      if (MODEL == 0) {
+        s_flux[it] = make_float4(F[0], F[1], F[2], F[3]);
+      } else {
+        s_flux[it * 3 + 0] = make_float4(F[0], F[1], F[2], F[3]);
+        s_flux[it * 3 + 1] = make_float4(F[4 % NF], F[5 % NF], F[6 % NF], F[7 % NF]);
+        s_flux[it * 3 + 2] = make_float4(F[8 % NF], 0.f, 0.f, 0.f);
+      }
+      continue;
+    }
     const int nm = p.fmask[j];
     const int nb = s_nbr[e * 4 + f];
     const float *qm = s_q + (e * NF) * NP + nm;

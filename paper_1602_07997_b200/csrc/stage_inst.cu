@@ -3,6 +3,7 @@
 #include "kernels.cuh"
 #include "tc3_kernels.cuh"
 #include "epk_kernels.cuh"
+#include "iface_kernels.cuh"
 
 #if !defined(DG_MODEL) || !defined(DG_N)
 #error "compile with -DDG_MODEL=0|1 -DDG_N=1..10"
@@ -62,6 +63,11 @@ extern "C" int DG_CAT3(dgk_tc3_info_, DG_MODEL, DG_N)(int what) {
     case 10: return C::PT;
     default: return -1;
   }
+}
+
+// interface-centric surface kernel (iface_kernels.cuh)
+extern "C" const void *DG_CAT3(dgk_get_iface_kernel_, DG_MODEL, DG_N)(void) {
+  return (const void *)&dgk::iface_flux_kernel<DG_MODEL, DG_N>;
 }
 
 #ifdef DG_PROF

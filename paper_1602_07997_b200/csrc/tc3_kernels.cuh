@@ -642,6 +642,28 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
 #pragma unroll 1
       for (int h = 0; h < C::NHC; ++h, ++fc) {
         const int fs = fc % NFL, fuse = fc / NFL;
+        if (p.pflux) {
+          // interface-centric surface step (iface_kernels.cuh): the chunk's penalty terms are already in the face buffer
+          // [K][Nf][4 Nfp]; rows (element, field) x FCH face nodes are copied into the ring slot, coalesced along the nodes
+          constexpr int RPI = T3_FLUXW * 32 / C::FCH;                 // rows per pass
+          const int jj = ft % C::FCH, j = C::FCH * h + jj;
+          float v[(128 + RPI - 1) / RPI];
+#pragma unroll
+          for (int i = 0; i < (128 + RPI - 1) / RPI; ++i) {
+            const int row = ft / C::FCH + RPI * i;
+            v[i] = (j < NFACE && row < nvalid * NF) ? __ldg(p.pflux + ((size_t)k0 * NF + row) * NFACE + j) : 0.f;
+          }
+          T3_WAIT(flEmpty(fs), (fuse & 1) ^ 1, 1);
+          float *fl = s_flux + fs * (128 * C::FLS);
+#pragma unroll
+          for (int i = 0; i < (128 + RPI - 1) / RPI; ++i) {
+            const int row = ft / C::FCH + RPI * i;
+            if (row < 128) fl[row * C::FLS + jj] = v[i];
+          }
+          __syncwarp();
+          if (lane == 0) tc::mbar_arrive(flFull(fs));
+          continue;
+        }
         // ---- this thread's tasks of the chunk: one face node jj of the chunk, elements e0, e0 + EPI, ... (the face, the
         // interior node and the row of the neighbour-node table are the same for all of them)
         constexpr int EPI = T3_FLUXW * 32 / C::FCH;   // element stride between a thread's tasks

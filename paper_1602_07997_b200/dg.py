@@ -31,12 +31,15 @@ class _Materials(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("device", C.c_int), ("variant", C.c_int), ("elems_per_thread", C.c_int), ("groups_per_cta", C.c_int),
-                ("max_ctas", C.c_int)]
+                ("max_ctas", C.c_int), ("surface", C.c_int), ("owned_elements", C.c_int64)]
 
 
 EXPORTS = ["dg_create", "dg_destroy", "dg_num_fields", "dg_np", "dg_nfp", "dg_num_elements", "dg_node_coords",
            "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_stage", "dg_stage_range", "dg_range_alignment", "dg_element_dt", "dg_ab3_step", "dg_ab3_run", "dg_ab3_reset", "dg_last_launch_count",
-           "dg_variant_name", "dg_reference_operators", "dg_geometry", "dg_connectivity", "dg_last_error"]
+           "dg_variant_name", "dg_reference_operators", "dg_geometry", "dg_connectivity", "dg_last_error",
+           "dg_partition_create", "dg_partition_destroy", "dg_partition_num_owned", "dg_partition_num_ghost",
+           "dg_partition_global_ids", "dg_partition_local_mesh", "dg_partition_num_peers", "dg_partition_peer",
+           "dg_partition_halo_faces", "dg_halo_pack", "dg_halo_unpack", "dg_num_owned_elements"]
 
 _lib.dg_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(_Materials), C.POINTER(_Options)]
 _lib.dg_create.restype = C.c_int
@@ -65,6 +68,18 @@ _lib.dg_reference_operators.argtypes = [C.c_void_p] + [C.c_void_p] * 6
 _lib.dg_geometry.argtypes = [C.c_void_p] + [C.c_void_p] * 4
 _lib.dg_connectivity.argtypes = [C.c_void_p] + [C.c_void_p] * 3
 _lib.dg_last_error.restype = C.c_char_p
+_lib.dg_partition_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Mesh), C.c_int, C.c_int]
+_lib.dg_partition_destroy.argtypes = [C.c_void_p]
+for _n in ("dg_partition_num_owned", "dg_partition_num_ghost", "dg_num_owned_elements"):
+    getattr(_lib, _n).argtypes = [C.c_void_p]
+    getattr(_lib, _n).restype = C.c_int64
+_lib.dg_partition_global_ids.argtypes = [C.c_void_p, C.c_void_p]
+_lib.dg_partition_local_mesh.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.dg_partition_num_peers.argtypes = [C.c_void_p]
+_lib.dg_partition_peer.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+_lib.dg_partition_halo_faces.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+_lib.dg_halo_pack.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+_lib.dg_halo_unpack.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
 
 
 class DGError(RuntimeError):
@@ -90,7 +105,7 @@ class Context:
     """dg_create / dg_destroy pair.  Host arrays are numpy; device buffers are raw pointers (ints)."""
 
     def __init__(self, vxyz, etov, N: int, model: int, rho, c_or_vp, vs=None, bc=None, device: int = 0,
-                 elems_per_thread: int = 0, groups_per_cta: int = 0, variant: int = 0, max_ctas: int = 0):
+                 elems_per_thread: int = 0, groups_per_cta: int = 0, variant: int = 0, max_ctas: int = 0, surface: int = 0, owned_elements: int = 0):
         vxyz = np.ascontiguousarray(vxyz, dtype=np.float64)
         etov = np.ascontiguousarray(etov, dtype=np.int32)
         bc = None if bc is None else np.ascontiguousarray(bc, dtype=np.int8)
@@ -99,13 +114,14 @@ class Context:
         vs = None if vs is None else np.ascontiguousarray(vs, dtype=np.float64)
         mesh = _Mesh(vxyz.shape[0], etov.shape[0], _ptr(vxyz), _ptr(etov), _ptr(bc))
         mat = _Materials(_ptr(rho), _ptr(c_or_vp), _ptr(vs))
-        opt = _Options(device, variant, elems_per_thread, groups_per_cta, max_ctas)
+        opt = _Options(device, variant, elems_per_thread, groups_per_cta, max_ctas, surface, owned_elements)
         h = C.c_void_p()
         self._h = None
         _check(_lib.dg_create(C.byref(h), C.byref(mesh), int(N), int(model), C.byref(mat), C.byref(opt)))
         self._h = h
         self.N, self.model, self.device = int(N), int(model), device
         self.K = int(_lib.dg_num_elements(h))
+        self.K_owned = int(_lib.dg_num_owned_elements(h))
         self.Np, self.Nfp, self.NF = int(_lib.dg_np(h)), int(_lib.dg_nfp(h)), int(_lib.dg_num_fields(h))
 
     # -- lifetime
@@ -198,6 +214,12 @@ class Context:
         _check(_lib.dg_element_dt(self._h, float(cfl), _ptr(out)))
         return out
 
+    def halo_pack(self, d_q: int, d_faces: int, nfaces: int, d_buf: int, stream: int | None = None):
+        _check(_lib.dg_halo_pack(self._h, C.c_void_p(d_q), C.c_void_p(d_faces), int(nfaces), C.c_void_p(d_buf), C.c_void_p(stream or 0)))
+
+    def halo_unpack(self, d_q: int, d_faces: int, nfaces: int, d_buf: int, stream: int | None = None):
+        _check(_lib.dg_halo_unpack(self._h, C.c_void_p(d_q), C.c_void_p(d_faces), int(nfaces), C.c_void_p(d_buf), C.c_void_p(stream or 0)))
+
     def ab3_step(self, d_q: int, dt: float, stream: int | None = None):
         _check(_lib.dg_ab3_step(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))
 
@@ -206,6 +228,44 @@ class Context:
 
     def ab3_reset(self, stream: int | None = None):
         _check(_lib.dg_ab3_reset(self._h, C.c_void_p(stream or 0)))
+
+
+class Partition:
+    """dg_partition_*: one rank's slab of the element list, its ghost elements and the halo face lists per peer."""
+
+    def __init__(self, vxyz, etov, bc, nranks: int, rank: int):
+        vxyz = np.ascontiguousarray(vxyz, dtype=np.float64)
+        etov = np.ascontiguousarray(etov, dtype=np.int32)
+        bc = None if bc is None else np.ascontiguousarray(bc, dtype=np.int8)
+        mesh = _Mesh(vxyz.shape[0], etov.shape[0], _ptr(vxyz), _ptr(etov), _ptr(bc))
+        h = C.c_void_p()
+        self._h = None
+        _check(_lib.dg_partition_create(C.byref(h), C.byref(mesh), int(nranks), int(rank)))
+        self._h = h
+        self.nranks, self.rank = int(nranks), int(rank)
+        self.num_owned = int(_lib.dg_partition_num_owned(h))
+        self.num_ghost = int(_lib.dg_partition_num_ghost(h))
+        n = self.num_owned + self.num_ghost
+        self.global_ids = np.empty(n, dtype=np.int64)
+        _check(_lib.dg_partition_global_ids(h, _ptr(self.global_ids)))
+        self.etov = np.empty((n, 4), dtype=np.int32)
+        self.bc = np.empty((n, 4), dtype=np.int8)
+        _check(_lib.dg_partition_local_mesh(h, _ptr(self.etov), _ptr(self.bc)))
+        self.peers = []                      # (peer rank, send faces, recv faces): 4 * local element + face
+        for i in range(int(_lib.dg_partition_num_peers(h))):
+            r, ns, nr = C.c_int(), C.c_int64(), C.c_int64()
+            _check(_lib.dg_partition_peer(h, i, C.byref(r), C.byref(ns), C.byref(nr)))
+            send, recv = np.empty(ns.value, dtype=np.int32), np.empty(nr.value, dtype=np.int32)
+            _check(_lib.dg_partition_halo_faces(h, i, _ptr(send), _ptr(recv)))
+            self.peers.append((r.value, send, recv))
+
+    def close(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.dg_partition_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
 
 
 def from_workload(w, device: int = 0, **opts) -> Context:

@@ -280,3 +280,96 @@ def test_stage_range_is_refused_on_padded_rows(dg):
     o = torch.zeros_like(d)
     with pytest.raises(dg.DGError):
         case.ctx.stage_range(d.data_ptr(), o.data_ptr(), 0.0, 1.0, 1e-3, 0, case.ctx.K)
+
+
+# ---------------------------------------------------------------- interface-centric surface step
+@pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 1, {}), (W.ELASTIC, 1, {}), (W.ACOUSTIC, 2, {}), (W.ELASTIC, 2, {}),
+                                          (W.ACOUSTIC, 3, {}), (W.ELASTIC, 3, {"max_ctas": 2}), (W.ACOUSTIC, 5, {"max_ctas": 2}),
+                                          (W.ELASTIC, 4, {}), (W.ELASTIC, 7, {}), (W.ACOUSTIC, 10, {"max_ctas": 4}),
+                                          (W.ACOUSTIC, 3, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1})])
+def test_interface_centric_surface_step(dg, model, N, opts):
+    """dg_options.surface = 1: the paper's SGEMM-strategy surface kernel -- one thread per interface face node computes the
+    penalty terms of both sides once into a face buffer, boundary faces behind the interior ones -- as the producer of rows
+    a4 + a5 for each stage-kernel family (element per thread, tensor core, fused SIMT): r(q), two LSRK steps and five AB3
+    steps against the oracle, and against the element-centric default (same formulas per side: agreement to rounding)."""
+    w = _sweep_case(model, N)
+    w.top = W.BC_SLIP if model == W.ELASTIC else W.BC_FREE          # rigid, and free / slip faces among the boundary ones
+    case = Case(dg, w, surface=1, **opts)
+    assert "interface-centric" in case.ctx.variant_name
+    q32 = case.initial_fields32()
+    q64 = q32.astype(np.float64)
+    got = case.gpu_rhs(torch, q32)
+    assert case.ctx.last_launch_count in (2, 4)                      # interface kernel + stage kernel (+ two layout conversions)
+    assert_close(got, case.oracle_rhs(q64), RHS_TOL, f"{case.ctx.variant_name}: r(q)")
+    ref = Case(dg, w, **opts)
+    base = ref.gpu_rhs(torch, q32)
+    assert rel_l2(got, base) <= 2e-7, (case.ctx.variant_name, rel_l2(got, base))
+    dt = case.dt32()
+    assert_close(case.gpu_run(torch, q32, dt, 2), case.oracle_run(q64, dt, 2), 1e-5, f"{case.ctx.variant_name}: two LSRK steps")
+    from oracle import timestep as ts
+    d_q = torch.from_numpy(q32).cuda()
+    dta = case.dt32(0.05)
+    case.ctx.ab3_run(d_q.data_ptr(), dta, 5)
+    torch.cuda.synchronize()
+    q, hist = q64.copy(), []
+    for _ in range(5):
+        ts.ab3_step(q, hist, dta, case.oracle_rhs)
+    assert_close(d_q.cpu().numpy(), q, 1e-5, f"{case.ctx.variant_name}: five AB3 steps")
+
+
+# ---------------------------------------------------------------- multi-GPU form on one GPU: two partitions, halo exchange
+@pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 1, {}), (W.ACOUSTIC, 3, {}), (W.ELASTIC, 4, {}), (W.ELASTIC, 6, {"max_ctas": 2}),
+                                          (W.ACOUSTIC, 9, {}), (W.ELASTIC, 2, {"variant": 1}), (W.ACOUSTIC, 3, {"surface": 1})])
+def test_two_partitions_with_halo_exchange_match_single_domain(dg, model, N, opts):
+    """The path as it would run on two GPUs, emulated rank after rank on one: each rank's context holds
+    its slab of the element list plus ghost copies (dg_partition_*, dg_options.owned_elements); before every LSRK stage the
+    face traces of the cut faces are packed (dg_halo_pack), handed to the peer (here: a device copy where NCCL send/recv
+    would be) and unpacked into its ghosts (dg_halo_unpack); dg_stage then advances the owned elements.  Two steps must
+    reproduce the single-domain result bit for bit -- ghosts start as NaN, so nothing but exchanged traces is ever read."""
+    w = _sweep_case(model, N)
+    vxyz, etov, bc, cell = w.mesh()
+    mats = w.material_arrays(cell)
+    single = Case(dg, w, **opts)
+    q32 = single.initial_fields32()
+    dt = single.dt32()
+    want = single.gpu_run(torch, q32, dt, 2)
+    stream = torch.cuda.current_stream().cuda_stream
+    ranks = []
+    for r in range(2):
+        part = dg.Partition(vxyz, etov, bc, 2, r)
+        ids, no = part.global_ids, part.num_owned
+        ctx = dg.Context(vxyz, part.etov, N, model, mats[0][ids], mats[1][ids], mats[2][ids] if model == W.ELASTIC else None,
+                         part.bc, device=0, owned_elements=no, **opts)
+        assert ctx.K_owned == no and ctx.K == len(ids) and part.num_ghost > 0
+        q = q32[ids].copy()
+        q[no:] = np.nan
+        cur = torch.from_numpy(q).cuda()
+        nxt = torch.full_like(cur, float("nan"))
+        peers = [(peer, torch.from_numpy(s).cuda(), torch.from_numpy(rv).cuda(),
+                  torch.empty(len(s) * ctx.NF * ctx.Nfp, device="cuda"), torch.empty(len(rv) * ctx.NF * ctx.Nfp, device="cuda"))
+                 for peer, s, rv in part.peers]
+        assert [p[0] for p in peers] == [1 - r]
+        ranks.append(dict(part=part, ctx=ctx, cur=cur, nxt=nxt, peers=peers))
+    for step in range(2):
+        for s in range(5):
+            for rk in ranks:                                       # pack on every rank
+                for peer, send, recv, sbuf, rbuf in rk["peers"]:
+                    rk["ctx"].halo_pack(rk["cur"].data_ptr(), send.data_ptr(), send.numel(), sbuf.data_ptr(), stream)
+            for r, rk in enumerate(ranks):                         # "send / recv": my receive buffer is the peer's send buffer
+                for peer, send, recv, sbuf, rbuf in rk["peers"]:
+                    other = [p for p in ranks[peer]["peers"] if p[0] == r][0]
+                    assert other[3].numel() == rbuf.numel()
+                    rbuf.copy_(other[3])
+                    rk["ctx"].halo_unpack(rk["cur"].data_ptr(), recv.data_ptr(), recv.numel(), rbuf.data_ptr(), stream)
+            for rk in ranks:
+                rk["ctx"].stage(rk["cur"].data_ptr(), rk["nxt"].data_ptr(), A[s], B[s], dt, stream)
+                rk["cur"], rk["nxt"] = rk["nxt"], rk["cur"]
+    torch.cuda.synchronize()
+    for rk in ranks:
+        ids, no = rk["part"].global_ids, rk["part"].num_owned
+        got = rk["cur"].cpu().numpy()[:no]
+        assert np.isfinite(got).all(), "a ghost value that was never exchanged reached an owned element"
+        assert np.array_equal(got, want[ids[:no]]), f"rank {rk['part'].rank}: {describe(got, want[ids[:no]])}"
+    halo_bytes = sum(4 * (p[3].numel() + p[4].numel()) for rk in ranks for p in rk["peers"])
+    state_bytes = 4 * q32.size
+    assert halo_bytes < state_bytes                                # only traces of the cut faces move
