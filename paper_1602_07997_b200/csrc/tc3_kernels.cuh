@@ -783,12 +783,8 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
       tc::tc_fence_after();
       const uint32_t d0 = tm + set * 2 * NCH, d1 = d0 + NCH;
       for (int st = 0; st < C::NSTEP; ++st) {
-#if defined(DG_X_W2) && !defined(DG_PROF)
-        tc::mbar_wait2(fullA(sa), pa, fullB(sb), pb);
-#else
         T3_WAIT(fullA(sa), pa, 1);
         T3_WAIT(fullB(sb), pb, 2);
-#endif
         tc::tc_fence_after();
         if (tc::elect_one()) {
           const uint32_t a1 = tm + C::ABASE + sa * T3_ASTRIDE, a2 = a1 + 8, a3 = a1 + 16;

@@ -29,22 +29,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "r"(parity), "r"(0x989680)       // suspend-time hint: the warp sleeps in hardware instead of spinning on issue slots
       : "memory");
 }
-// wait for two barriers whose probes are issued back to back (their latencies overlap; used by the MMA warp, which needs an
-// operand stage of each ring per k-step)
-__device__ __forceinline__ void mbar_wait2(uint32_t bar_a, uint32_t par_a, uint32_t bar_b, uint32_t par_b) {
-  asm volatile(
-      "{\n\t.reg .pred PA, PB;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 PA, [%0], %1;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 PB, [%2], %3;\n\t"
-      "WA:\n\t@PA bra DA;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 PA, [%0], %1, %4;\n\t"
-      "bra WA;\n\tDA:\n\t"
-      "WB:\n\t@PB bra DB;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 PB, [%2], %3, %4;\n\t"
-      "bra WB;\n\tDB:\n\t}\n" ::"r"(bar_a),
-      "r"(par_a), "r"(bar_b), "r"(par_b), "r"(0x989680)
-      : "memory");
-}
 // barrier among a subset of the CTA's warps (id 1..15; all `nthreads` threads must call it)
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
