@@ -12,7 +12,16 @@ The path scales weakly: per stage and rank the exchange moves Nfields * Nfp floa
 """
 from __future__ import annotations
 
+from fractions import Fraction
+
 import numpy as np
+
+# the 2N-storage coefficients dg_run uses (Carpenter & Kennedy; reading Q2), for drivers that go stage by stage
+LSRK_A = tuple(float(Fraction(*f)) for f in ((0, 1), (-567301805773, 1357537059087), (-2404267990393, 2016746695238),
+                                             (-3550918686646, 2091501179385), (-1275806237668, 842570457699)))
+LSRK_B = tuple(float(Fraction(*f)) for f in ((1432997174477, 9575080441755), (5161836677717, 13612068292357),
+                                             (1720146321549, 2090206949498), (3134564353537, 4481467310338),
+                                             (2277821191437, 14882151754819)))
 
 
 class HaloExchanger:
@@ -33,21 +42,49 @@ class HaloExchanger:
         return sum(4 * (p["sbuf"].numel() + p["rbuf"].numel()) for p in self.peers)
 
     def exchange(self, q, stream=None):
-        """q: device tensor [K_local][Nf][Np] (owned elements then ghosts).  Packs on `stream`, exchanges, unpacks."""
+        """q: device tensor [K_local][Nf][Np] (owned elements then ghosts).  Packs on `stream`, exchanges, unpacks.
+        With the NCCL backend the device buffers go out as they are (peer copies over NVLink); with gloo (tests: several
+        processes on one GPU or none) they are staged through host memory."""
         import torch.distributed as dist
         torch = self.torch
         sptr = stream.cuda_stream if stream is not None else None
         for p in self.peers:
             self.ctx.halo_pack(q.data_ptr(), p["send"].data_ptr(), p["send"].numel(), p["sbuf"].data_ptr(), sptr)
-        ops = []
+        staged = dist.get_backend(self.group) != "nccl"
+        if stream is not None:
+            stream.synchronize()                   # the packed buffers are complete before they leave
+        else:
+            torch.cuda.current_stream().synchronize()
+        ops, back = [], []
         for p in self.peers:
-            ops.append(dist.P2POp(dist.isend, p["sbuf"], p["rank"], group=self.group))
-            ops.append(dist.P2POp(dist.irecv, p["rbuf"], p["rank"], group=self.group))
+            sb = p["sbuf"].cpu() if staged else p["sbuf"]
+            rb = torch.empty(p["rbuf"].shape, dtype=p["rbuf"].dtype) if staged else p["rbuf"]
+            back.append((p, rb))
+            ops.append(dist.P2POp(dist.isend, sb, p["rank"], group=self.group))
+            ops.append(dist.P2POp(dist.irecv, rb, p["rank"], group=self.group))
         if ops:
             for w in dist.batch_isend_irecv(ops):
                 w.wait()
-        for p in self.peers:
+        for p, rb in back:
+            if staged:
+                p["rbuf"].copy_(rb)
             self.ctx.halo_unpack(q.data_ptr(), p["recv"].data_ptr(), p["recv"].numel(), p["rbuf"].data_ptr(), sptr)
+
+    def run_lsrk(self, q, dt: float, nsteps: int, stream=None):
+        """nsteps LSRK(5,4) steps of the partitioned mesh: per stage exchange the cut faces' traces, then dg_stage on the owned
+        elements (ping-pong between `q` and a scratch tensor; the result ends in `q`).  Coefficients: the library's
+        (dg_run's) Carpenter-Kennedy pairs, passed stage by stage."""
+        torch = self.torch
+        sptr = stream.cuda_stream if stream is not None else None
+        cur, nxt = q, torch.empty_like(q)
+        for _ in range(nsteps):
+            for a, b in zip(LSRK_A, LSRK_B):
+                self.exchange(cur, stream)
+                self.ctx.stage(cur.data_ptr(), nxt.data_ptr(), a, b, dt, sptr)
+                cur, nxt = nxt, cur
+        if cur is not q:
+            q.copy_(cur)
+        return q
 
 
 def pack_host(q: np.ndarray, faces: np.ndarray, fmask: np.ndarray) -> np.ndarray:
