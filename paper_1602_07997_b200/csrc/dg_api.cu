@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "../../include/dg.h"
+#include "dg_prof.h"
 #include "host_setup.hpp"
 #include "kernels.cuh"
 #include "tc3_kernels.cuh"
@@ -929,7 +930,7 @@ int dg_ab3_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
 int dg_ab3_step(dg_ctx *c, float *d_q, float dt, void *stream) { return dg_ab3_run(c, d_q, dt, 1, stream); }
 
 #ifdef DG_PROF
-// development builds only (-DDG_PROF): per-warp wait-cycle counters of the last variant-4 launch, [296][23][5] int64
+// development builds only (-DDG_PROF; declared in dg_prof.h, not in include/dg.h)
 int dg_prof_read(dg_ctx *c, long long *out) {
   typedef int (*rd)(long long *);
   static const rd R[2][11] = {DG_ROW(0, dgk_prof_read_), DG_ROW(1, dgk_prof_read_)};

@@ -185,3 +185,20 @@ def test_element_dt_levels_for_multirate(dg, refelems):
     levels = np.floor(np.log2(got / got.min())).astype(int)
     assert levels.max() >= 2 and (np.bincount(levels) > 0).sum() >= 3
     assert ctx.range_alignment in (1, 14, 32) or ctx.range_alignment > 0
+
+
+def test_option_values_are_validated(dg):
+    """dg_options: unknown variant / surface values, a negative max_ctas and owned_elements beyond K are DG_ERR_ARG."""
+    vxyz, etov, _ = W.kuhn_cube(1, 0.0)
+    one = np.ones(6)
+    for bad in (dict(variant=3), dict(surface=2), dict(max_ctas=-1), dict(owned_elements=7)):
+        with pytest.raises(dg.DGError) as e:
+            dg.Context(vxyz, etov, 2, dg.ACOUSTIC, one, one, device=-1, **bad)
+        assert e.value.code == -1, bad
+    ok = dg.Context(vxyz, etov, 2, dg.ACOUSTIC, one, one, device=-1, owned_elements=4, surface=1, max_ctas=3)
+    assert ok.K == 6 and ok.K_owned == 4
+    for call in (lambda: ok.stage(16, 32, 0.0, 1.0, 1e-3), lambda: ok.stage_range(16, 32, 0.0, 1.0, 1e-3, 0, 4),
+                 lambda: ok.ab3_run(16, 1e-3, 2), lambda: ok.halo_pack(16, 32, 1, 48), lambda: ok.halo_unpack(16, 32, 1, 48)):
+        with pytest.raises(dg.DGError) as e:
+            call()
+        assert e.value.code == -4 and "no CPU fallback" in str(e.value)
