@@ -124,7 +124,7 @@ class ClockSampler:
         """Statistics of the rows since the last mark(); the sampler keeps running."""
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         rows = self.rows[self.first:] or self.rows[-1:]
         for r in rows:
@@ -132,10 +132,15 @@ class ClockSampler:
                 sm.append(float(r[0])); mx.append(float(r[1]))
             except (ValueError, IndexError):
                 continue
+            try:
+                pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                pass
             for nme, v in zip(names, r[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(nme)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_min_mhz": min(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "power_w": statistics.median(pw) if pw else None,
                 "samples": len(sm), "reasons": sorted(reasons)}
 
     def stop(self):
@@ -443,6 +448,11 @@ def run_ours(a):
     roof = roofline_of(ctx.variant_name, w.model, w.N, w.K, t_stage, a.integrator)
     tensor = ctx.variant_name.startswith("tc_")
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    # the first run after the (idle) set-up runs at full boost, the later ones under the board's power cap: both are shown
+    t_first = ms_list[0] * 1e-3 / stages
+    first = roofline_of(ctx.variant_name, w.model, w.N, w.K, t_first, a.integrator)
+    roof["first_run"] = {"ms_per_stage": t_first * 1e3, "frac": first["frac"], "note": "first of the timed runs (boost clocks); "
+                         "`frac` above is the median run (sustained, power-capped)"}
     roof["traffic"] = None
     if os.path.exists(tpath) and not ab3:
         roof["traffic"] = json.load(open(tpath)).get(w.name + (":tc" if tensor else ":simt"))
