@@ -373,3 +373,36 @@ def test_two_partitions_with_halo_exchange_match_single_domain(dg, model, N, opt
     halo_bytes = sum(4 * (p[3].numel() + p[4].numel()) for rk in ranks for p in rk["peers"])
     state_bytes = 4 * q32.size
     assert halo_bytes < state_bytes                                # only traces of the cut faces move
+
+
+# ---------------------------------------------------------------- full size: the optional paths, kernel against kernel
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_size_ab3_and_interface_paths_every_element(dg, cfg):
+    """BASELINE.json sizes: (1) six steps of the paper's AB3 integrator (two start-up steps, four fused AB3 kernels; 81 / 78
+    batches per persistent CTA) on the tensor-core kernel against the fused SIMT kernel, which the small-mesh tests pin to
+    the oracle; (2) two LSRK steps with the interface-centric surface kernel against the element-centric default.  Every
+    element is compared."""
+    w = W.config(cfg)
+    outs = {}
+    q32 = dt = None
+    for name, opts, what in (("tc_ab3", {"variant": 4}, "ab3"), ("simt_ab3", {"variant": 1}, "ab3"),
+                             ("tc", {"variant": 4}, "lsrk"), ("tc_iface", {"variant": 4, "surface": 1}, "lsrk")):
+        ctx = dg.from_workload(w, device=0, **opts)
+        if q32 is None:
+            q32 = w.initial_fields(ctx.node_coords()).astype(np.float32)
+            dt = float(np.float32(ctx.stable_dt(0.5)))
+        d = torch.from_numpy(q32).cuda()
+        if what == "ab3":
+            ctx.ab3_run(d.data_ptr(), 0.1 * dt, 6)
+        else:
+            ctx.run(d.data_ptr(), dt, 2)
+        torch.cuda.synchronize()
+        outs[name] = d
+        ctx.close()
+    d0 = torch.from_numpy(q32).cuda()
+    for a, b in (("tc_ab3", "simt_ab3"), ("tc_iface", "tc")):
+        diff = (outs[a] - outs[b]).double()
+        err = float(diff.norm() / outs[b].double().norm())
+        inc = float(diff.norm() / (outs[b] - d0).double().norm())
+        worst = int(diff.abs().amax(dim=(1, 2)).argmax())
+        assert err <= 1e-5 and inc <= 2e-4, f"{w.name}: {a} vs {b}: rel-L2 {err:.3e}, of the increment {inc:.3e}, worst element {worst}"
