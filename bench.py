@@ -496,12 +496,12 @@ def run_ours(a):
         if not a.no_cpu and world == 1:
             per_stage_flop = flops_per_element(w.model, w.N)
             sample_elems = a.sample or max(256, int(2.0e9 / per_stage_flop / 5))
-            times, threads, desc, ns = oracle_sample_run(w, 2, sample_elems)
-            sec = times[-1]
+            times, threads, desc, ns = oracle_sample_run(w, 6, sample_elems)      # ~10 s of CPU work; the first step is warm-up
+            sec = statistics.mean(times[1:])
             line["cpu_baseline"] = {"value": ns * w.Np * 5 / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
                                     "sample": desc, "net_gflops_fp64": ns * per_stage_flop * 5 / sec * 1e-9}
-            t1, _, d1, n1 = oracle_sample_run(w, 1, max(128, sample_elems // 4), threads=1)
-            line["cpu_baseline"]["single_thread"] = {"value": n1 * w.Np * 5 / t1[-1], "unit": UNIT, "cores": 1, "sample": d1}
+            t1, _, d1, n1 = oracle_sample_run(w, 4, max(128, sample_elems // 4), threads=1)
+            line["cpu_baseline"]["single_thread"] = {"value": n1 * w.Np * 5 / statistics.mean(t1[1:]), "unit": UNIT, "cores": 1, "sample": d1}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
