@@ -45,8 +45,14 @@ struct EpkFmask {
   }
 };
 
+// resident CTAs per SM asked of the compiler: the kernel is bound by the latency of its scattered gathers, so occupancy pays
+// as long as the register cap does not spill much (same-box A/B, ms per stage: acoustic N = 1 0.752 -> 0.713 with six CTAs;
+// elastic N = 1 1.772 -> 1.658 and acoustic N = 2 0.801 -> 0.789 with four; five or six CTAs there spill and lose 12-75 %)
+template <int MODEL, int N>
+constexpr int epk_min_ctas() { return (MODEL == 0 && N == 1) ? 6 : 4; }
+
 template <int MODEL, int N, int MODE>
-__global__ void __launch_bounds__(128) epk_stage_kernel(const StageParams p) {
+__global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kernel(const StageParams p) {
   using D = Deg<N>;
   constexpr int NP = D::NP, NFP = D::NFP, NFACE = D::NFACE;
   constexpr int NF = MODEL == 0 ? 4 : 9, NGEO = MODEL == 0 ? GEO_AC : GEO_EL;
