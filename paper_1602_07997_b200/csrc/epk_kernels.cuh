@@ -59,8 +59,13 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   constexpr int NV = NF * NP;                                          // values per element
   static_assert(NV % 4 == 0, "an element's fields are moved as 16-byte vectors");
   constexpr EpkFmask<N> FM{};
-  const int k = p.kbeg + blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= p.K) return;
+  // N = 1, acoustic: an element is four 16-byte vectors (one per field), and the four lanes of a quad gather their
+  // neighbours' elements together (below): every lane stays alive, lanes beyond the range redo the last element and store nothing
+  constexpr bool COOP = NP == 4 && MODEL == 0;
+  const int k_raw = p.kbeg + blockIdx.x * blockDim.x + threadIdx.x;
+  if (!COOP && k_raw >= p.K) return;
+  const bool active = k_raw < p.K;
+  const int k = active ? k_raw : p.K - 1;
 
   // ---- per-element constants and fields
   // the element's record: G[9], materials, 4 face records -- whole in registers for the acoustic model (32 values),
@@ -171,6 +176,9 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   }
 
   // ---- surface term (rows a4-a6): gather, penalty terms times g^sur, lift
+  // the element's connectivity as two vector loads (the kernel is bound by its load / store instructions, not by DRAM)
+  const int4 nbr4 = __ldg(reinterpret_cast<const int4 *>(p.nbr) + k);
+  const unsigned code4 = __ldg(reinterpret_cast<const unsigned *>(p.fcode) + k);
 #pragma unroll
   for (int f = 0; f < 4; ++f) {
     constexpr int FO = MODEL == 0 ? 12 : 16, FS = MODEL == 0 ? 5 : 8;
@@ -178,16 +186,30 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
 #pragma unroll
     for (int i = 0; i < FS; ++i) fg[i] = MODEL == 0 ? gl[(FO + FS * f + i) % NGL] : __ldg(g + FO + FS * f + i);
     const float nx = fg[0], ny = fg[1], nz = fg[2];
-    const int nb = __ldg(p.nbr + (size_t)k * 4 + f);
-    const int code = (int)__ldg(p.fcode + (size_t)k * 4 + f);
+    const int nb = f == 0 ? nbr4.x : (f == 1 ? nbr4.y : (f == 2 ? nbr4.z : nbr4.w));      // (f is a compile-time constant: unrolled)
+    const int code = (int)((code4 >> (8 * f)) & 255u);
     // N = 1: a field of the neighbour is one 16-byte vector (Np = 4): fetch it whole and pick the node afterwards
     // (a third of the gather instructions; the kernel is bound by the L1/LSU pipe, the ALUs are idle)
-    constexpr bool VGATHER = NP == 4 && MODEL == 0;              // (elastic N = 1: nine vectors per face cost more registers than they save)
+    constexpr bool VGATHER = COOP;                               // (elastic N = 1: nine vectors per face cost more registers than they save)
     float4 nq[VGATHER ? NF : 1];
-    if (VGATHER && nb >= 0 && !p.pflux) {
-      const float4 *src = reinterpret_cast<const float4 *>(p.q_in + (size_t)nb * NV);
+    if (VGATHER && !p.pflux) {
+      // Warp-level gather: the kernel is bound by the L1 tag stage (one 128-byte line per lane and load: 32 lines per warp
+      // instruction).  Lane j of a quad loads vector j (= field j) of the neighbour of each of the quad's four elements in
+      // turn -- 8 lines per warp instruction instead of 32 -- and the quad transposes the 4 x 4 vectors through a padded
+      // shared-memory row per lane (conflict-free 16-byte accesses).
+      __shared__ float4 s_x[128 * 5];
+      const int lane = threadIdx.x & 31, qj = lane & 3, qb = lane & ~3;
 #pragma unroll
-      for (int c = 0; c < NF; ++c) nq[c] = __ldg(src + c);
+      for (int i = 0; i < 4; ++i) {
+        const int nbi = __shfl_sync(0xffffffffu, nb, qb + i);
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (nbi >= 0) v = __ldg(reinterpret_cast<const float4 *>(p.q_in + (size_t)nbi * NV) + qj);
+        s_x[((threadIdx.x & ~3) + i) * 5 + qj] = v;
+      }
+      __syncwarp();
+#pragma unroll
+      for (int c = 0; c < NF; ++c) nq[c] = s_x[threadIdx.x * 5 + c];
+      __syncwarp();
     }
     auto pick = [](const float4 &v, int nn) { return (nn & 2) ? ((nn & 1) ? v.w : v.z) : ((nn & 1) ? v.y : v.x); };
 #pragma unroll
@@ -254,6 +276,7 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   }
 
   // ---- LSRK update (row a7), 16-byte vectors
+  if (!active) return;                                                 // (lanes kept alive for the quad gather only)
   const size_t base = (size_t)k * NV;
   if (MODE == MODE_RHS) {
     float4 *dst = reinterpret_cast<float4 *>(p.rhs + base);
