@@ -478,10 +478,10 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         pend = -1;
       }
     };
-    auto emit = [&](const float *a) {
+    auto emit = [&](const float2 *a) {
       uint32_t p1[4], p2[4], p3[4];
 #pragma unroll
-      for (int t = 0; t < 4; ++t) tc::split3(a[2 * t], a[2 * t + 1], p1[t], p2[t], p3[t]);
+      for (int t = 0; t < 4; ++t) tc::split3(a[t], p1[t], p2[t], p3[t]);
       finish();
       T3_WAIT(emptyA(slot), phase ^ 1, 0);
       tc::tc_fence_after();
@@ -521,7 +521,13 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         // mean of the four vertex values: D_j 1 = 0, so the shift is exact and removes the cancellation
         mean[i] = (valid && i < nsrc) ? 0.25f * ((ldq(sp[i]) + ldq(sp[i] + N)) + (ldq(sp[i] + C::NFP - 1) + ldq(sp[i] + NP - 1))) : 0.f;
       }
-      auto load_u = [&](int g, float (&u)[3][8]) {
+      // (packed FP32 arithmetic on register pairs from here on: FADD2 / FMUL2 / FFMA2)
+      auto shifted = [&](const float4 &v, int i, float2 &lo, float2 &hi) {
+        const float2 nm = make_float2(-mean[i], -mean[i]);
+        lo = __fadd2_rn(make_float2(v.x, v.y), nm);
+        hi = __fadd2_rn(make_float2(v.z, v.w), nm);
+      };
+      auto load_u = [&](int g, float2 (&u)[3][4]) {
         const int m0 = 16 * g + 8 * half;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
@@ -531,20 +537,19 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
               if (m0 + 4 * h4 < NP) {
                 const float4 v = TILE ? *reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4)
                                       : __ldg(reinterpret_cast<const float4 *>(sp[i] + m0 + 4 * h4));
-                u[i][4 * h4 + 0] = v.x - mean[i]; u[i][4 * h4 + 1] = v.y - mean[i];
-                u[i][4 * h4 + 2] = v.z - mean[i]; u[i][4 * h4 + 3] = v.w - mean[i];
+                shifted(v, i, u[i][2 * h4], u[i][2 * h4 + 1]);
               } else {
-                u[i][4 * h4 + 0] = u[i][4 * h4 + 1] = u[i][4 * h4 + 2] = u[i][4 * h4 + 3] = 0.f;
+                u[i][2 * h4] = u[i][2 * h4 + 1] = make_float2(0.f, 0.f);
               }
             }
           } else {
 #pragma unroll
-            for (int t = 0; t < 8; ++t) u[i][t] = 0.f;
+            for (int t = 0; t < 4; ++t) u[i][t] = make_float2(0.f, 0.f);
           }
         }
       };
       // without a tile the loader streams the fields as chunks of 16 nodes x 128 rows (64 B swizzle) through a ring
-      auto load_u_ring = [&](int g, const unsigned char *ring, float (&u)[3][8]) {
+      auto load_u_ring = [&](int g, const unsigned char *ring, float2 (&u)[3][4]) {
         const int m0 = 16 * g + 8 * half;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
@@ -556,21 +561,20 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
             for (int h4 = 0; h4 < 2; ++h4) {
               if (m0 + 4 * h4 < NP) {
                 const float4 v = *reinterpret_cast<const float4 *>(rowp + (((2 * half + h4) ^ sw) << 4));
-                u[i][4 * h4 + 0] = v.x - mean[i]; u[i][4 * h4 + 1] = v.y - mean[i];
-                u[i][4 * h4 + 2] = v.z - mean[i]; u[i][4 * h4 + 3] = v.w - mean[i];
+                shifted(v, i, u[i][2 * h4], u[i][2 * h4 + 1]);
               } else {
-                u[i][4 * h4 + 0] = u[i][4 * h4 + 1] = u[i][4 * h4 + 2] = u[i][4 * h4 + 3] = 0.f;
+                u[i][2 * h4] = u[i][2 * h4 + 1] = make_float2(0.f, 0.f);
               }
             }
           } else {
 #pragma unroll
-            for (int t = 0; t < 8; ++t) u[i][t] = 0.f;
+            for (int t = 0; t < 4; ++t) u[i][t] = make_float2(0.f, 0.f);
           }
         }
       };
 #pragma unroll 1
       for (int g = 0; g < C::NG; ++g) {
-        float u[3][8];
+        float2 u[3][4];
         if (TILE) {
           load_u(g, u);
         } else {
@@ -583,9 +587,10 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         }
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-          float a[8];
+          const float2 c0 = make_float2(cf[j][0], cf[j][0]), c1 = make_float2(cf[j][1], cf[j][1]), c2 = make_float2(cf[j][2], cf[j][2]);
+          float2 a[4];
 #pragma unroll
-          for (int t = 0; t < 8; ++t) a[t] = cf[j][0] * u[0][t] + cf[j][1] * u[1][t] + cf[j][2] * u[2][t];
+          for (int t = 0; t < 4; ++t) a[t] = __ffma2_rn(c2, u[2][t], __ffma2_rn(c1, u[1][t], __fmul2_rn(c0, u[0][t])));
           emit(a);
         }
       }
@@ -597,15 +602,15 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
         constexpr int KPC = C::FCH / 16;                              // k-steps per flux chunk
         if (h % KPC == 0) T3_WAIT(flFull(fs), fuse & 1, 2);
         const float *fl = s_flux + fs * (128 * C::FLS) + r * C::FLS + 16 * (h % KPC) + 8 * half;
-        float a[8];
+        float2 a[4];
         if (valid) {
           const float4 v0 = *reinterpret_cast<const float4 *>(fl);
           const float4 v1 = *reinterpret_cast<const float4 *>(fl + 4);
           // (columns beyond 4 Nfp hold zeros or finite penalty terms of an earlier chunk: the operator rows there are zero)
-          a[0] = v0.x; a[1] = v0.y; a[2] = v0.z; a[3] = v0.w; a[4] = v1.x; a[5] = v1.y; a[6] = v1.z; a[7] = v1.w;
+          a[0] = make_float2(v0.x, v0.y); a[1] = make_float2(v0.z, v0.w); a[2] = make_float2(v1.x, v1.y); a[3] = make_float2(v1.z, v1.w);
         } else {
 #pragma unroll
-          for (int t = 0; t < 8; ++t) a[t] = 0.f;
+          for (int t = 0; t < 4; ++t) a[t] = make_float2(0.f, 0.f);
         }
         if (h % KPC == KPC - 1 || h == C::NH - 1) {                   // done with the chunk
           __syncwarp();

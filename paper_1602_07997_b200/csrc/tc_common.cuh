@@ -89,5 +89,16 @@ __device__ __forceinline__ void split3(float x0, float x1, uint32_t &p1, uint32_
   const float t0 = r0 - __uint_as_float(p2 << 16), t1 = r1 - __uint_as_float(p2 & 0xFFFF0000u);
   p3 = pack_bf16(t0, t1);
 }
+// the same on a register pair with the packed FP32 instructions of sm_100 (FFMA2: two lanes per issue slot; the
+// tensor-core kernel is bound by its warps' instruction issue, not by the FMA pipe).  x - hi is exact either way.
+__device__ __forceinline__ float2 unpack_bf16(uint32_t p) { return make_float2(__uint_as_float(p << 16), __uint_as_float(p & 0xFFFF0000u)); }
+__device__ __forceinline__ void split3(float2 x, uint32_t &p1, uint32_t &p2, uint32_t &p3) {
+  const float2 m1 = make_float2(-1.f, -1.f);
+  p1 = pack_bf16(x.x, x.y);
+  const float2 r = __ffma2_rn(unpack_bf16(p1), m1, x);
+  p2 = pack_bf16(r.x, r.y);
+  const float2 t = __ffma2_rn(unpack_bf16(p2), m1, r);
+  p3 = pack_bf16(t.x, t.y);
+}
 }  // namespace tc
 }  // namespace dgk
