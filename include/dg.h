@@ -81,7 +81,9 @@ typedef struct {
                                  thread for acoustic N <= 2 / elastic N = 1, fused node per thread otherwise or when
                                  elems_per_thread / groups_per_cta is given);
                                  4 = pipelined warp-specialised tensor-core kernel (tcgen05, BF16x3 split, TMEM
-                                 accumulators), every degree; needs 16-byte aligned q / rhs and K < 2^26.
+                                 accumulators), every degree; needs 16-byte aligned q / rhs and K < 2^26;
+                                 5 = FP32 SIMT row-per-thread kernel (thread = (element, field), operators in
+                                 constant memory), N <= 3 (DG_ERR_ARG above); needs 16-byte aligned q / rhs.
                                  Any other value: DG_ERR_ARG                                           */
   int elems_per_thread;       /* 0 = auto; register blocking E of the SIMT kernel (1..8)         */
   int groups_per_cta;         /* 0 = auto; node groups G per CTA (CTA handles G*E elements)      */

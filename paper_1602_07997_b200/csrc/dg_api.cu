@@ -28,7 +28,10 @@
   extern "C" const void *dgk_get_epk_kernel_##m##_##n(int);       \
   extern "C" int dgk_epk_upload_##m##_##n(const float *, const float *, const unsigned short *, const int *); \
   extern "C" const void *dgk_get_iface_kernel_##m##_##n(void);   \
-  extern "C" int dgk_tc3_info_##m##_##n(int);
+  extern "C" int dgk_tc3_info_##m##_##n(int);                     \
+  extern "C" const void *dgk_get_rpt_kernel_##m##_##n(int);       \
+  extern "C" int dgk_rpt_info_##m##_##n(int);                     \
+  extern "C" int dgk_rpt_upload_##m##_##n(const float *, const float *);
 #define DG_DECL_ALL(m) \
   DG_DECL(m, 1) DG_DECL(m, 2) DG_DECL(m, 3) DG_DECL(m, 4) DG_DECL(m, 5) DG_DECL(m, 6) DG_DECL(m, 7) DG_DECL(m, 8) DG_DECL(m, 9) DG_DECL(m, 10)
 DG_DECL_ALL(0)
@@ -56,6 +59,10 @@ const tc_getter EPK_KERNELS[2][11] = {DG_ROW(0, dgk_get_epk_kernel_), DG_ROW(1, 
 const epk_upload_fn EPK_UPLOAD[2][11] = {DG_ROW(0, dgk_epk_upload_), DG_ROW(1, dgk_epk_upload_)};
 const tc_getter TC3_KERNELS[2][11] = {DG_ROW(0, dgk_get_tc3_kernel_), DG_ROW(1, dgk_get_tc3_kernel_)};
 const info_getter TC3_INFO[2][11] = {DG_ROW(0, dgk_tc3_info_), DG_ROW(1, dgk_tc3_info_)};
+typedef int (*rpt_upload_fn)(const float *, const float *);
+const tc_getter RPT_KERNELS[2][11] = {DG_ROW(0, dgk_get_rpt_kernel_), DG_ROW(1, dgk_get_rpt_kernel_)};
+const info_getter RPT_INFO[2][11] = {DG_ROW(0, dgk_rpt_info_), DG_ROW(1, dgk_rpt_info_)};
+const rpt_upload_fn RPT_UPLOAD[2][11] = {DG_ROW(0, dgk_rpt_upload_), DG_ROW(1, dgk_rpt_upload_)};
 typedef const void *(*iface_getter)(void);
 const iface_getter IFACE_KERNELS[2][11] = {DG_ROW(0, dgk_get_iface_kernel_), DG_ROW(1, dgk_get_iface_kernel_)};
 
@@ -125,6 +132,8 @@ struct dg_ctx {
   unsigned short *d_fmask = nullptr, *d_nbrnode = nullptr;
   uint16_t *d_Bimg = nullptr;                    // tensor-core variant: bf16x3 operator panel image
   bool tc3 = false;                              // pipelined BF16x3 tensor-core variant (tc3_kernels.cuh)
+  bool rpt = false;                              // row-per-thread kernel (rpt_kernels.cuh): N <= 3
+  int rpt_epc = 0;                               // its elements per CTA
   bool epk = false;                              // element-per-thread kernel (epk_kernels.cuh): acoustic N <= 2, elastic N = 1
   int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
   int epi_cw = 0;                                // tc3: epilogue chunk width (TMA box columns)
@@ -284,7 +293,24 @@ void choose_variant(dg_ctx *c, const dg_options *o) {
   // auto (config-4 sweep): the tensor-core kernel from N = 3 up and for elastic N = 2; at N = 1 (Np = 4:
   // three of four k-steps are padding) and acoustic N = 2 the fused SIMT kernel with one element per thread is faster
   if (want == 0) want = ((c->N >= 3 || (c->N == 2 && c->model == DG_ELASTIC)) && c->K < (1 << 26)) ? 4 : 1;
-  if (want != 1 && want != 4) throw std::invalid_argument("unknown variant (0 auto, 1 fused FP32 SIMT, 4 pipelined tensor core BF16x3)");
+  if (want != 1 && want != 4 && want != 5)
+    throw std::invalid_argument("unknown variant (0 auto, 1 fused FP32 SIMT, 4 pipelined tensor core BF16x3, 5 FP32 SIMT row per thread)");
+  if (want == 5) {
+    if (!RPT_KERNELS[c->model][c->N](dgk::MODE_STAGE)) throw std::invalid_argument("the row-per-thread variant covers N <= 3");
+    c->rpt = true;
+    c->k_rhs = RPT_KERNELS[c->model][c->N](dgk::MODE_RHS);
+    c->k_stage = RPT_KERNELS[c->model][c->N](dgk::MODE_STAGE);
+    c->k_ab3 = RPT_KERNELS[c->model][c->N](dgk::MODE_AB3);
+    c->NT = RPT_INFO[c->model][c->N](0);
+    c->rpt_epc = RPT_INFO[c->model][c->N](1);
+    c->smem = 0;
+    c->grid = (int)((c->K_active + c->rpt_epc - 1) / c->rpt_epc);
+    char buf[160];
+    snprintf(buf, sizeof buf, "simt_row_per_thread<%s,N=%d,threads=%d,elems/cta=%d,operators in constant memory>",
+             c->model == DG_ACOUSTIC ? "acoustic" : "elastic", c->N, c->NT, c->rpt_epc);
+    c->variant = buf;
+    return;
+  }
   if (want == 4) {
     if (c->K >= (1 << 26)) throw std::invalid_argument("pipelined tensor-core variant packs the neighbour in 26 bits: K < 2^26");
     c->tc3 = true;
@@ -399,7 +425,7 @@ std::array<CUtensorMap, 5> tensor_maps(dg_ctx *c, const void *ptr, bool pin = fa
 // elements per unit of work of the chosen kernel: element ranges of dg_stage_range start on multiples of it
 int range_alignment(const dg_ctx *c) {
   if (c->tc3) return TC3_INFO[c->model][c->N](1);
-  if (c->epk) return 1;
+  if (c->epk || c->rpt) return 1;
   return c->G * c->E;
 }
 
@@ -428,12 +454,12 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   }
   int grid = c->grid;
   if (kbeg != 0 || kend != c->K_active) {
-    const int unit = c->epk ? 128 : range_alignment(c);
+    const int unit = c->epk ? 128 : (c->rpt ? c->rpt_epc : range_alignment(c));
     grid = (int)((kend - kbeg + unit - 1) / unit);
   }
   dgk::Tc3Params tp3;
   void *args[] = {&p};
-  if (c->epk && (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15))
+  if ((c->epk || c->rpt) && (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15))
     return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
   if (c->tc3) {
     if (((uintptr_t)q_in | (uintptr_t)q_out | (uintptr_t)rhs) & 15) return fail(DG_ERR_ARG, "device buffers must be 16-byte aligned");
@@ -567,6 +593,17 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
         std::vector<int> fm(c->ref.fmask.begin(), c->ref.fmask.end());
         const int rc = EPK_UPLOAD[c->model][c->N](Dm.data(), Lm.data(), nbrnode.data(), fm.data());
         if (rc == -1) throw std::runtime_error("element-per-thread kernel: face masks differ from the compile-time table");
+        if (rc != 0) throw std::runtime_error(std::string("cuda: ") + cudaGetErrorString((cudaError_t)rc) + " uploading the operators to constant memory");
+      }
+      if (c->rpt) {
+        std::vector<float> Dt((size_t)3 * Np * Np), Lt((size_t)4 * Nfp * Np);
+        const std::vector<double> *Ds3[3] = {&c->ref.Dr, &c->ref.Ds, &c->ref.Dt};
+        for (int m = 0; m < Np; ++m)
+          for (int d = 0; d < 3; ++d)
+            for (int n = 0; n < Np; ++n) Dt[((size_t)3 * m + d) * Np + n] = (float)(*Ds3[d])[(size_t)n * Np + m];
+        for (int j = 0; j < 4 * Nfp; ++j)
+          for (int n = 0; n < Np; ++n) Lt[(size_t)j * Np + n] = (float)c->ref.LIFT[(size_t)n * 4 * Nfp + j];
+        const int rc = RPT_UPLOAD[c->model][c->N](Dt.data(), Lt.data());
         if (rc != 0) throw std::runtime_error(std::string("cuda: ") + cudaGetErrorString((cudaError_t)rc) + " uploading the operators to constant memory");
       }
       if (c->tc3) {

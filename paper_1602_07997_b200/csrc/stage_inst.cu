@@ -4,6 +4,7 @@
 #include "tc3_kernels.cuh"
 #include "epk_kernels.cuh"
 #include "iface_kernels.cuh"
+#include "rpt_kernels.cuh"
 
 #if !defined(DG_MODEL) || !defined(DG_N)
 #error "compile with -DDG_MODEL=0|1 -DDG_N=1..10"
@@ -103,6 +104,40 @@ extern "C" int DG_CAT3(dgk_epk_upload_, DG_MODEL, DG_N)(const float *D, const fl
   return (int)e;
 #else
   (void)D; (void)L; (void)nbrnode; (void)fmask;
+  return -2;
+#endif
+}
+
+// row-per-thread kernel (rpt_kernels.cuh): N <= 3; NULL otherwise
+#define DG_HAS_RPT (DG_N <= 3)
+extern "C" const void *DG_CAT3(dgk_get_rpt_kernel_, DG_MODEL, DG_N)(int mode) {
+#if DG_HAS_RPT
+  if (mode == dgk::MODE_RHS) return (const void *)&dgk::rpt_stage_kernel<DG_MODEL, DG_N, dgk::MODE_RHS>;
+  if (mode == dgk::MODE_STAGE) return (const void *)&dgk::rpt_stage_kernel<DG_MODEL, DG_N, dgk::MODE_STAGE>;
+  if (mode == dgk::MODE_AB3) return (const void *)&dgk::rpt_stage_kernel<DG_MODEL, DG_N, dgk::MODE_AB3>;
+#endif
+  (void)mode;
+  return nullptr;
+}
+// what = 0 threads per CTA, 1 elements per CTA
+extern "C" int DG_CAT3(dgk_rpt_info_, DG_MODEL, DG_N)(int what) {
+#if DG_HAS_RPT
+  using C = dgk::Rpt<DG_MODEL, DG_N>;
+  return what == 0 ? C::WARPS * 32 : (what == 1 ? C::EPC : -1);
+#else
+  (void)what;
+  return -1;
+#endif
+}
+// uploads the operators into this translation unit's constant memory: DT [m][j][n] = D_j[n][m], LT [j][n] = LIFT[n][j]
+extern "C" int DG_CAT3(dgk_rpt_upload_, DG_MODEL, DG_N)(const float *DT, const float *LT) {
+#if DG_HAS_RPT
+  using Dg = dgk::Deg<DG_N>;
+  cudaError_t e = cudaMemcpyToSymbol(dgk::c_rpt_D, DT, sizeof(float) * 3 * Dg::NP * Dg::NP);
+  if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_rpt_L, LT, sizeof(float) * Dg::NP * Dg::NFACE);
+  return (int)e;
+#else
+  (void)DT; (void)LT;
   return -2;
 #endif
 }

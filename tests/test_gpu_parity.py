@@ -46,6 +46,21 @@ def test_rhs_parity_all_degrees(dg, variant, model, N):
     assert max(per_field) <= 2 * RHS_TOL, (per_field, describe(got, want))
 
 
+@pytest.mark.parametrize("N", range(1, 4))
+@pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
+def test_rhs_parity_row_per_thread(dg, model, N):
+    """Variant 5 (rpt_kernels.cuh: thread = (element, field) row, operators in constant memory), N = 1..3: the same case as
+    above -- ragged last warp (K = 162 is no multiple of 8 or 3), boundary faces of both kinds -- against the oracle."""
+    case = Case(dg, _sweep_case(model, N), variant=5)
+    assert case.ctx.variant_name.startswith("simt_row_per_thread")
+    q32 = case.initial_fields32()
+    got = case.gpu_rhs(torch, q32)
+    want = case.oracle_rhs(q32.astype(np.float64))
+    assert_close(got, want, RHS_TOL, case.ctx.variant_name)
+    per_field = [rel_l2(got[:, f], want[:, f]) for f in range(got.shape[1])]
+    assert max(per_field) <= 2 * RHS_TOL, (per_field, describe(got, want))
+
+
 @pytest.mark.parametrize("model,N,E,G", [(W.ACOUSTIC, 1, 1, 16), (W.ACOUSTIC, 2, 1, 5), (W.ACOUSTIC, 3, 8, 3), (W.ACOUSTIC, 4, 2, 1),
                                          (W.ELASTIC, 1, 2, 8), (W.ELASTIC, 2, 4, 7), (W.ELASTIC, 3, 1, 2), (W.ELASTIC, 5, 4, 1)])
 def test_rhs_parity_other_launch_shapes(dg, model, N, E, G):
@@ -182,7 +197,8 @@ def test_zero_field_gives_zero_rhs_and_energy_decays(dg):
 
 
 @pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 3, {}), (W.ELASTIC, 5, {"max_ctas": 2}), (W.ELASTIC, 8, {}), (W.ACOUSTIC, 2, {}),
-                                          (W.ELASTIC, 1, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 10, {"max_ctas": 4})])
+                                          (W.ELASTIC, 1, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 10, {"max_ctas": 4}),
+                                          (W.ACOUSTIC, 3, {"variant": 5}), (W.ELASTIC, 2, {"variant": 5})])
 def test_ab3_matches_paper_eq4(dg, model, N, opts):
     """The paper's own integrator (eq. (4)) as a fused epilogue of every stage-kernel family: 24 steps
     (two start-up steps, reading Q21, then 22 fused AB3 kernels -- with `max_ctas` several batches per persistent
@@ -257,6 +273,8 @@ def test_variant_selection_and_errors(dg):
     assert names[(W.ACOUSTIC, 3)].startswith("tc_pipe") and names[(W.ELASTIC, 3)].startswith("tc_pipe")
     with pytest.raises(dg.DGError):
         Case(dg, _sweep_case(W.ACOUSTIC, 3, n=1), variant=2)
+    with pytest.raises(dg.DGError):                                  # the row-per-thread kernel stops at N = 3
+        Case(dg, _sweep_case(W.ACOUSTIC, 4, n=1), variant=5)
     case = Case(dg, _sweep_case(W.ACOUSTIC, 3, n=1), variant=4)
     buf = torch.zeros(int(np.prod(case.ctx.shape)) + 1, dtype=torch.float32, device="cuda")
     out = torch.zeros_like(buf)

@@ -71,6 +71,24 @@ def test_run_parity_every_degree_auto(dg, model, N):
     assert_close(three, case.oracle_run(q64, dt, 3), RUN_TOL, f"{case.ctx.variant_name}: three LSRK steps")
 
 
+@pytest.mark.parametrize("N", range(1, 4))
+@pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
+def test_run_parity_row_per_thread(dg, model, N):
+    """The same trajectory check for variant 5 (row-per-thread kernel, N <= 3): one LSRK step to 2e-6 with the increment
+    check, three steps to 1e-4."""
+    case = Case(dg, _sweep_case(model, N), variant=5)
+    assert case.ctx.variant_name.startswith("simt_row_per_thread")
+    q32 = case.initial_fields32()
+    q64 = q32.astype(np.float64)
+    dt = case.dt32()
+    one = case.gpu_run(torch, q32, dt, 1)
+    want1 = case.oracle_run(q64, dt, 1)
+    assert_close(one, want1, RHS_TOL, f"{case.ctx.variant_name}: one LSRK step")
+    inc = _increment_error(one, want1, q64)
+    assert inc <= 2e-5, f"{case.ctx.variant_name}: increment of one step off by {inc:.3e}; {describe(one, want1)}"
+    assert_close(case.gpu_run(torch, q32, dt, 3), case.oracle_run(q64, dt, 3), RUN_TOL, f"{case.ctx.variant_name}: three LSRK steps")
+
+
 # ---------------------------------------------------------------- persistent CTAs over several batches (tensor-core kernel)
 @pytest.mark.parametrize("N", range(1, 11))
 @pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
@@ -231,7 +249,8 @@ def test_element_per_thread_vs_node_per_thread_every_element(dg, model, N):
 
 # ---------------------------------------------------------------- multi-rate hook: a stage restricted to an element range
 @pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 1, {}), (W.ACOUSTIC, 3, {}), (W.ELASTIC, 3, {}), (W.ELASTIC, 5, {"max_ctas": 2}),
-                                          (W.ELASTIC, 9, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1})])
+                                          (W.ELASTIC, 9, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1}),
+                                          (W.ACOUSTIC, 3, {"variant": 5}), (W.ELASTIC, 2, {"variant": 5})])
 def test_stage_range_composes_to_the_full_stage(dg, model, N, opts):
     """dg_stage_range over [0, k1), [k1, k2), [k2, K) -- the per-level launches of a multi-rate driver
     -- writes exactly what one dg_stage over the mesh writes, touches nothing outside its range (q_out and the residual),
@@ -286,11 +305,12 @@ def test_stage_range_is_refused_on_padded_rows(dg):
 @pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 1, {}), (W.ELASTIC, 1, {}), (W.ACOUSTIC, 2, {}), (W.ELASTIC, 2, {}),
                                           (W.ACOUSTIC, 3, {}), (W.ELASTIC, 3, {"max_ctas": 2}), (W.ACOUSTIC, 5, {"max_ctas": 2}),
                                           (W.ELASTIC, 4, {}), (W.ELASTIC, 7, {}), (W.ACOUSTIC, 10, {"max_ctas": 4}),
-                                          (W.ACOUSTIC, 3, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1})])
+                                          (W.ACOUSTIC, 3, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1}),
+                                          (W.ACOUSTIC, 2, {"variant": 5}), (W.ELASTIC, 3, {"variant": 5})])
 def test_interface_centric_surface_step(dg, model, N, opts):
     """dg_options.surface = 1: the paper's SGEMM-strategy surface kernel -- one thread per interface face node computes the
     penalty terms of both sides once into a face buffer, boundary faces behind the interior ones -- as the producer of rows
-    a4 + a5 for each stage-kernel family (element per thread, tensor core, fused SIMT): r(q), two LSRK steps and five AB3
+    a4 + a5 for each stage-kernel family (element per thread, tensor core, fused SIMT, row per thread): r(q), two LSRK steps and five AB3
     steps against the oracle, and against the element-centric default (same formulas per side: agreement to rounding)."""
     w = _sweep_case(model, N)
     w.top = W.BC_SLIP if model == W.ELASTIC else W.BC_FREE          # rigid, and free / slip faces among the boundary ones
