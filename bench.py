@@ -536,7 +536,7 @@ def main():
     ap.add_argument("--sample", type=int, default=None, help="elements in the oracle's timed sample")
     ap.add_argument("--E", type=int, default=0)
     ap.add_argument("--G", type=int, default=0)
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 fused FP32 SIMT kernel, 4 pipelined tcgen05 BF16x3 kernel")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 FP32 SIMT family, 4 pipelined tcgen05 BF16x3 kernel, 5 FP32 SIMT row-per-thread kernel (N <= 3)")
     ap.add_argument("--surface", default="element", choices=["element", "interface"],
                     help="interface: the paper's interface-centric surface kernel feeds the stage kernel (dg_options.surface = 1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

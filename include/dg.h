@@ -77,7 +77,7 @@ typedef struct {              /* HOST, per element, fp64 (piecewise-constant med
 typedef struct {
   int device;                 /* CUDA device ordinal; -1 = host-only context (setup introspection,
                                  no device entry point works: they return DG_ERR_CUDA)           */
-  int variant;                /* 0 = auto (1 for N = 1 and acoustic N = 2, else 4); 1 = FP32 SIMT stage kernels (element per
+  int variant;                /* 0 = auto (1 for N = 1, 5 for N = 2, else 4); 1 = FP32 SIMT stage kernels (element per
                                  thread for acoustic N <= 2 / elastic N = 1, fused node per thread otherwise or when
                                  elems_per_thread / groups_per_cta is given);
                                  4 = pipelined warp-specialised tensor-core kernel (tcgen05, BF16x3 split, TMEM

@@ -133,7 +133,8 @@ struct dg_ctx {
   uint16_t *d_Bimg = nullptr;                    // tensor-core variant: bf16x3 operator panel image
   bool tc3 = false;                              // pipelined BF16x3 tensor-core variant (tc3_kernels.cuh)
   bool rpt = false;                              // row-per-thread kernel (rpt_kernels.cuh): N <= 3
-  int rpt_epc = 0;                               // its elements per CTA
+  int rpt_epc = 0;                               // its elements per CTA and tile round
+  int rpt_cap = 0;                               // its persistent grid: resident CTAs per SM x SMs (set at the first launch)
   bool epk = false;                              // element-per-thread kernel (epk_kernels.cuh): acoustic N <= 2, elastic N = 1
   int *d_conn = nullptr;                         // tc3: packed connectivity [K][4]
   int epi_cw = 0;                                // tc3: epilogue chunk width (TMA box columns)
@@ -290,9 +291,14 @@ void build_tc3_image(const dgh::RefElem &ref, int NCH, int nsplit, int nstep, st
 
 void choose_variant(dg_ctx *c, const dg_options *o) {
   int want = o ? o->variant : 0;
-  // auto (config-4 sweep): the tensor-core kernel from N = 3 up and for elastic N = 2; at N = 1 (Np = 4:
-  // three of four k-steps are padding) and acoustic N = 2 the fused SIMT kernel with one element per thread is faster
-  if (want == 0) want = ((c->N >= 3 || (c->N == 2 && c->model == DG_ELASTIC)) && c->K < (1 << 26)) ? 4 : 1;
+  // auto (config-4 sweep): the tensor-core kernel from N = 3 up; the row-per-thread kernel at N = 2
+  // (acoustic 0.74 vs 0.79 ms element per thread; elastic 1.98 vs 2.62 ms tensor core); the element-per-thread kernel at N = 1
+  // (Np = 4: three of four k-steps of the tensor-core kernel would be padding) -- an explicit launch shape asks for the
+  // fused node-per-thread kernel
+  if (want == 0) {
+    const bool shape = o && (o->elems_per_thread > 0 || o->groups_per_cta > 0);
+    want = shape ? 1 : ((c->N >= 3 && c->K < (1 << 26)) ? 4 : (c->N == 2 ? 5 : 1));
+  }
   if (want != 1 && want != 4 && want != 5)
     throw std::invalid_argument("unknown variant (0 auto, 1 fused FP32 SIMT, 4 pipelined tensor core BF16x3, 5 FP32 SIMT row per thread)");
   if (want == 5) {
@@ -456,6 +462,16 @@ int launch_stage(dg_ctx *c, const void *kernel, const float *q_in, float *q_out,
   if (kbeg != 0 || kend != c->K_active) {
     const int unit = c->epk ? 128 : (c->rpt ? c->rpt_epc : range_alignment(c));
     grid = (int)((kend - kbeg + unit - 1) / unit);
+  }
+  if (c->rpt) {                                  // persistent warps: no more CTAs than the device holds at once
+    if (c->rpt_cap == 0) {
+      int per_sm = 0, sms = 0;
+      cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, c->k_stage, c->NT, 0);
+      if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+      if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " sizing the row-per-thread grid");
+      c->rpt_cap = std::max(1, per_sm) * std::max(1, sms);
+    }
+    grid = std::min(grid, c->max_ctas > 0 ? std::min(c->rpt_cap, c->max_ctas) : c->rpt_cap);
   }
   dgk::Tc3Params tp3;
   void *args[] = {&p};

@@ -10,9 +10,11 @@
 // immediate constant-bank operand, consecutive FFMAs walk consecutive constant addresses, and no operator value passes
 // through the load/store pipe (the generic fused kernel, kernels.cuh, is bound by exactly that traffic at these degrees;
 // the tensor-core kernel spends three of four k-steps on padding at N = 2 and pays its BF16x3 split per value).
-// The lanes of a warp are the Nf rows of 8 (acoustic) / 3 (elastic; 27 of 32 lanes) consecutive elements.  The warp stages
-// the fields of its elements in a shared-memory tile (coalesced, odd row pitch); pre-combination sources, interior traces
-// and the own row are read from there.  The 4 Nfp face nodes of an element are shared out over its Nf lanes (a4, a5:
+// The lanes of a warp are the Nf rows of 8 (acoustic) / 3 (elastic; 27 of 32 lanes) consecutive elements: a tile.  Warps are
+// persistent and work alone (no CTA-wide barrier): each walks over tiles with two shared-memory slots, the next tile's
+// fields, geometric records and connectivity landing through cp.async (4 bytes each: odd row pitches keep the scalar reads
+// conflict-free) while the current one is worked on; pre-combination sources, interior traces and the own row are read
+// from the slot.  The 4 Nfp face nodes of an element are shared out over its Nf lanes (a4, a5:
 // gather through the compressed connectivity, penalty terms of flux.cuh), pass through a second tile, and each lane lifts
 // its own field.  The arithmetic (vertex-mean shift, row coefficients, penalty terms) is the one of the other two families.
 //
@@ -50,7 +52,7 @@ struct Rpt {
   static constexpr int TPL = (NFACE + NF - 1) / NF;        // face nodes per lane
   static constexpr int VW = NP % 4 == 0 ? 4 : (NP % 2 == 0 ? 2 : 1);   // vector width of row accesses (floats)
   static constexpr int GP = NGEO | 1;                      // pitch of a geometric record in the tile: odd
-  static constexpr int WARPS = (32 * NPP + 32 * FP + EPW * GP) * 4 * 4 <= 48 * 1024 ? 4 : 2;   // warps per CTA (static shared memory)
+  static constexpr int WARPS = N <= 2 ? 2 : 1;                          // warps per CTA (each warp works alone; static shared memory < 48 KB)
   static constexpr int EPC = WARPS * EPW;                  // elements per CTA
 };
 
@@ -63,10 +65,18 @@ struct RptVec<2> { using T = float2; };
 template <>
 struct RptVec<1> { using T = float; };
 
-// resident CTAs per SM asked of the compiler (same-box A/B, ms per stage: acoustic N = 2 0.822 -> 0.759 with eight CTAs of
-// 64 registers; N = 3 1.04 -> 1.17 / 1.35 with six / eight: its 40 exterior-trace values in flight need the registers)
+// resident CTAs per SM asked of the compiler (same-box A/B, ms per stage, persistent version: N = 2 eight CTAs of two warps
+// and 128 registers -- acoustic 0.743, elastic 1.98; N = 3 twelve CTAs of one warp -- acoustic 1.15, elastic 3.21, against
+// 1.58 / 4.23 with two warps and no register cap: 200+ registers leave five warps per SM)
 template <int N>
-constexpr int rpt_min_ctas() { return N <= 2 ? 8 : 1; }
+constexpr int rpt_min_ctas() { return N <= 2 ? 8 : 12; }
+
+__device__ __forceinline__ void rpt_cp_async4(void *smem, const void *gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void rpt_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NKEEP>
+__device__ __forceinline__ void rpt_cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NKEEP) : "memory"); }
 
 template <int MODEL, int N, int MODE>
 __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) rpt_stage_kernel(const StageParams p) {
@@ -74,37 +84,68 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
   constexpr int NP = C::NP, NFP = C::NFP, NFACE = C::NFACE, NF = C::NF, NGEO = C::NGEO;
   constexpr int EPW = C::EPW, NPP = C::NPP, FP = C::FP, TPL = C::TPL, VW = C::VW;
   using Vec = typename RptVec<VW>::T;
-  __shared__ float s_qt[C::WARPS][32 * NPP];
+  // per warp: two slots of {fields, geometric records, connectivity} (the next tile lands while this one is worked on)
+  // and one tile of penalty terms
+  __shared__ float s_qt[C::WARPS][2][32 * NPP];
+  __shared__ float s_gt[C::WARPS][2][EPW * C::GP];
+  __shared__ int s_ct[C::WARPS][2][EPW * 5];                             // nbr [EPW][4], then fcode [EPW] (four bytes each)
   __shared__ float s_ft[C::WARPS][32 * FP];
-  __shared__ float s_gt[C::WARPS][EPW * C::GP];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int ke0 = p.kbeg + (blockIdx.x * C::WARPS + w) * EPW;
-  if (ke0 >= p.K) return;
-  const int nel = min(EPW, p.K - ke0);
-  float *sq = s_qt[w], *sf = s_ft[w], *sg = s_gt[w];
+  const int ntiles = (p.K - p.kbeg + EPW - 1) / EPW;
+  const int nwarps = gridDim.x * C::WARPS;
+  float *sf = s_ft[w];
 
-  // ---- the warp's fields -> tile (one contiguous run of nel Nf Np values; consecutive lanes, consecutive banks)
-  {
-    const int total = nel * NF * NP;
-    const float *src = p.q_in + (size_t)ke0 * NF * NP;
+  // tile -> slot, asynchronously (cp.async, 4 bytes each: the tiles have odd row pitches); one group per tile
+  auto issue = [&](int tile, int slot) {
+    const int ke0 = p.kbeg + tile * EPW;
+    const int nel = min(EPW, p.K - ke0);
+    {
+      const float *src = p.q_in + (size_t)ke0 * NF * NP;               // one contiguous run of nel Nf Np values
+      float *dst = s_qt[w][slot];
 #pragma unroll
-    for (int it = 0; it < (EPW * NF * NP + 31) / 32; ++it) {
-      const int idx = it * 32 + lane;
-      if (idx < total) {
-        const int row = idx / NP;
-        sq[idx + row * (NPP - NP)] = __ldg(src + idx);
+      for (int it = 0; it < (EPW * NF * NP + 31) / 32; ++it) {
+        const int idx = it * 32 + lane;
+        if (idx < nel * NF * NP) rpt_cp_async4(dst + idx + idx / NP * (NPP - NP), src + idx);
       }
     }
-  }
-  // ---- and their geometric records (G, materials, face records)
-  {
-    const float *src = p.geo + (size_t)ke0 * NGEO;
+    {
+      const float *src = p.geo + (size_t)ke0 * NGEO;
+      float *dst = s_gt[w][slot];
 #pragma unroll
-    for (int it = 0; it < (EPW * NGEO + 31) / 32; ++it) {
-      const int idx = it * 32 + lane;
-      if (idx < nel * NGEO) sg[idx + idx / NGEO * (C::GP - NGEO)] = __ldg(src + idx);
+      for (int it = 0; it < (EPW * NGEO + 31) / 32; ++it) {
+        const int idx = it * 32 + lane;
+        if (idx < nel * NGEO) rpt_cp_async4(dst + idx + idx / NGEO * (C::GP - NGEO), src + idx);
+      }
     }
+    {
+      int *dst = s_ct[w][slot];
+#pragma unroll
+      for (int it = 0; it < (EPW * 5 + 31) / 32; ++it) {
+        const int idx = it * 32 + lane;
+        if (idx < nel * 4) rpt_cp_async4(dst + idx, p.nbr + (size_t)ke0 * 4 + idx);
+        else if (idx >= EPW * 4 && idx < EPW * 4 + nel)
+          rpt_cp_async4(dst + idx, reinterpret_cast<const int *>(p.fcode) + ke0 + (idx - EPW * 4));
+      }
+    }
+    rpt_cp_commit();
+  };
+
+  int tile = blockIdx.x * C::WARPS + w;
+  if (tile < ntiles) issue(tile, 0);
+#pragma unroll 1
+  for (int it = 0; tile < ntiles; tile += nwarps, ++it) {
+  const int slot = it & 1;
+  if (tile + nwarps < ntiles) {
+    issue(tile + nwarps, slot ^ 1);
+    rpt_cp_wait<1>();
+  } else {
+    rpt_cp_wait<0>();
   }
+  __syncwarp();                                                          // (this tile's slot is complete, for every lane)
+  const int ke0 = p.kbeg + tile * EPW;
+  const int nel = min(EPW, p.K - ke0);
+  const float *sq = s_qt[w][slot], *sg = s_gt[w][slot];
+  const int *sc = s_ct[w][slot];
 
   // lanes without a row (elastic: 27 of 32; ragged last warp) follow row 0 and store nothing
   const bool valid = lane < nel * NF;
@@ -112,21 +153,22 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
   const int el = row / NF, f = row - el * NF;
   const int k = ke0 + el;
   const float *g = sg + el * C::GP;
+  const size_t base = ((size_t)k * NF + f) * NP;
 
   // ---- exterior traces of this lane's share of the element's face nodes (row a4): every load is issued here, without
-  // a branch in between, so that the whole chain connectivity -> neighbour node -> values is in flight behind the
-  // volume term (a lane with no task at t, or a boundary face, reads a valid address and ignores the value)
+  // a branch in between, so that the chain neighbour node -> values is in flight behind the volume term (a lane with no
+  // task at t, or a boundary face, reads a valid address and ignores the value)
   constexpr int TG = TPL * NF <= 48 ? TPL : 48 / NF;     // tasks whose traces are fetched ahead (register budget)
   int nbt[TPL];
   float up[TG][NF];
 #pragma unroll
   for (int t = 0; t < TPL; ++t) {
     const int j = min(f + NF * t, NFACE - 1), face = j / NFP;
-    nbt[t] = __ldg(p.nbr + (size_t)k * 4 + face);
+    nbt[t] = sc[el * 4 + face];
   }
   auto fetch = [&](int t, float (&x)[NF]) {
     const int j = min(f + NF * t, NFACE - 1), face = j / NFP, i = j - face * NFP;
-    const int code = __ldg(p.fcode + (size_t)k * 4 + face);
+    const int code = (sc[EPW * 4 + el] >> (8 * face)) & 255;
     const int nn = __ldg(p.nbrnode + (face * 24 + code) * NFP + i);
     const float *qp = p.q_in + (size_t)(nbt[t] >= 0 ? nbt[t] : k) * NF * NP + nn;
 #pragma unroll
@@ -136,7 +178,18 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
 #pragma unroll
     for (int t = 0; t < TG; ++t) fetch(t, up[t]);
   }
-  __syncwarp();                                                          // (the tiles are complete)
+  // the residual of this row (LSRK stage with A_s != 0): fetched here, used in the update
+  constexpr bool RESPF = MODE == MODE_STAGE;
+  float ores[RESPF ? NP : 1];
+  if (RESPF && p.a != 0.f) {
+#pragma unroll
+    for (int n = 0; n < NP; n += VW) {
+      const Vec v = *reinterpret_cast<const Vec *>(p.res + base + n);
+      if constexpr (VW == 4) { ores[n] = v.x; ores[n + 1] = v.y; ores[n + 2] = v.z; ores[n + 3] = v.w; }
+      else if constexpr (VW == 2) { ores[n] = v.x; ores[n + 1] = v.y; }
+      else { ores[n] = v; }
+    }
+  }
 
   // ---- volume term (rows a1-a3)
   float cf[3][3];
@@ -232,10 +285,8 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
       for (int n = 0; n < NP; ++n) r[n] = fmaf(c_rpt_L[j * NP + n], Fj, r[n]);
     }
   }
-  if (!valid) return;
-
   // ---- LSRK update (row a7), rows as vectors of VW values
-  const size_t base = ((size_t)k * NF + f) * NP;
+  if (valid) {
   auto ldv = [&](const float *ptr, int n, float (&x)[VW]) {
     const Vec v = *reinterpret_cast<const Vec *>(ptr + n);
     if constexpr (VW == 4) { x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
@@ -270,7 +321,12 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
       for (int t = 0; t < VW; ++t) rs[t] = p.dt * rr[t];
       if (p.a != 0.f) {
         float o[VW];
-        ldv(p.res + base, n, o);
+        if (RESPF) {
+#pragma unroll
+          for (int t = 0; t < VW; ++t) o[t] = ores[RESPF ? n + t : 0];
+        } else {
+          ldv(p.res + base, n, o);
+        }
 #pragma unroll
         for (int t = 0; t < VW; ++t) rs[t] = fmaf(p.a, o[t], rs[t]);
       }
@@ -279,6 +335,9 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
       for (int t = 0; t < VW; ++t) qq[t] = fmaf(p.b, rs[t], qq[t]);
       stv(p.q_out + base, n, qq);
     }
+  }
+  }
+  __syncwarp();                                                          // (every lane is done with this slot and the penalty tile)
   }
 }
 

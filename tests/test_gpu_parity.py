@@ -265,11 +265,11 @@ def test_padded_private_layout_paths(dg):
 
 
 def test_variant_selection_and_errors(dg):
-    """auto picks the element-per-thread SIMT kernel at N = 1 and acoustic N = 2, the tensor-core kernel elsewhere;
-    unknown variants and misaligned device buffers are rejected."""
+    """auto picks the element-per-thread SIMT kernel at N = 1, the row-per-thread one at N = 2, the tensor-core kernel
+    elsewhere; unknown variants and misaligned device buffers are rejected."""
     names = {(m, N): Case(dg, _sweep_case(m, N, n=1)).ctx.variant_name for m in (W.ACOUSTIC, W.ELASTIC) for N in (1, 2, 3)}
     assert names[(W.ACOUSTIC, 1)].startswith("simt_elem_per_thread") and names[(W.ELASTIC, 1)].startswith("simt_elem_per_thread")
-    assert names[(W.ACOUSTIC, 2)].startswith("simt_elem_per_thread") and names[(W.ELASTIC, 2)].startswith("tc_pipe")
+    assert names[(W.ACOUSTIC, 2)].startswith("simt_row_per_thread") and names[(W.ELASTIC, 2)].startswith("simt_row_per_thread")
     assert names[(W.ACOUSTIC, 3)].startswith("tc_pipe") and names[(W.ELASTIC, 3)].startswith("tc_pipe")
     with pytest.raises(dg.DGError):
         Case(dg, _sweep_case(W.ACOUSTIC, 3, n=1), variant=2)
@@ -284,7 +284,7 @@ def test_variant_selection_and_errors(dg):
 
 @pytest.mark.parametrize("model,N", [(W.ACOUSTIC, 1), (W.ACOUSTIC, 2), (W.ELASTIC, 1)])
 def test_element_per_thread_kernel_many_ctas(dg, model, N):
-    """The element-per-thread kernel (auto at these degrees) on a mesh of K = 162 000 elements (1 266 CTAs, ragged last
+    """The element-per-thread kernel (variant 1 at these degrees) on a mesh of K = 162 000 elements (1 266 CTAs, ragged last
     one): r_k on sampled elements against the oracle, and one LSRK step with non-increasing energy (its stage mode is
     compared with the oracle in test_gpu_stage_parity.py)."""
     from oracle import timestep
@@ -293,7 +293,7 @@ def test_element_per_thread_kernel_many_ctas(dg, model, N):
     K = w.K
     rng = np.random.default_rng(N)
     sample = np.unique(np.concatenate([np.arange(8), np.arange(K - 8, K), rng.integers(0, K, 48)]))
-    case = Case(dg, w, only_elems=sample)
+    case = Case(dg, w, only_elems=sample, variant=1)
     assert case.ctx.variant_name.startswith("simt_elem_per_thread")
     q32 = case.initial_fields32()
     got = case.gpu_rhs(torch, q32)[sample]

@@ -55,7 +55,7 @@ def _info(name, key):
 @pytest.mark.parametrize("model", [W.ACOUSTIC, W.ELASTIC])
 def test_run_parity_every_degree_auto(dg, model, N):
     """dg_run against oracle.timestep.lsrk_run for N = 1..10, both models, on the variant dg_create picks by itself
-    (element-per-thread SIMT kernel at N = 1 and acoustic N = 2, tensor-core kernel elsewhere): one step to 2e-6,
+    (element-per-thread SIMT kernel at N = 1, row-per-thread at N = 2, tensor-core kernel elsewhere): one step to 2e-6,
     three steps to 1e-4.  K = 162, random fields, random discontinuous materials, free top."""
     case = Case(dg, _sweep_case(model, N))
     q32 = case.initial_fields32()
@@ -192,10 +192,10 @@ def test_full_size_stage_mode_sampled(dg, cfg):
 
 @pytest.mark.parametrize("model,N", [(W.ACOUSTIC, 1), (W.ACOUSTIC, 2), (W.ELASTIC, 1)])
 def test_element_per_thread_stage_mode_sampled(dg, model, N):
-    """The element-per-thread kernel (auto at these degrees) in stage mode on K = 162 000 elements (1 266 CTAs)."""
+    """The element-per-thread kernel (variant 1 at these degrees) in stage mode on K = 162 000 elements (1 266 CTAs)."""
     w = W.config(4, N=N, model=model, n=30)
     w.ic = "random"
-    case = _two_stages_sampled(dg, w)
+    case = _two_stages_sampled(dg, w, variant=1)
     assert case.ctx.variant_name.startswith("simt_elem_per_thread")
 
 
@@ -232,7 +232,7 @@ def test_element_per_thread_vs_node_per_thread_every_element(dg, model, N):
     w = W.config(4, N=N, model=model, n=30)
     w.ic = "random"
     out = []
-    for opts in ({}, {"variant": 1, "elems_per_thread": 1}):
+    for opts in ({"variant": 1}, {"variant": 1, "elems_per_thread": 1}):
         ctx = dg.from_workload(w, device=0, **opts)
         if not out:
             q32 = w.initial_fields(ctx.node_coords()).astype(np.float32)
@@ -243,6 +243,37 @@ def test_element_per_thread_vs_node_per_thread_every_element(dg, model, N):
         out.append((ctx.variant_name, d))
         ctx.close()
     assert out[0][0].startswith("simt_elem_per_thread") and out[1][0].startswith("simt_fused")
+    err = float((out[0][1] - out[1][1]).double().norm() / out[1][1].double().norm())
+    assert err <= 1e-5, (out[0][0], out[1][0], err)
+
+
+@pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 2, {}), (W.ELASTIC, 2, {}), (W.ACOUSTIC, 3, {"variant": 5}), (W.ELASTIC, 1, {"variant": 5})])
+def test_row_per_thread_stage_mode_sampled(dg, model, N, opts):
+    """The row-per-thread kernel (auto at N = 2) in stage mode on K = 162 000 elements: every persistent warp walks over
+    several tiles through its two shared-memory slots (cp.async prefetch of the next tile), ragged last tile."""
+    w = W.config(4, N=N, model=model, n=30)
+    w.ic = "random"
+    case = _two_stages_sampled(dg, w, **opts)
+    assert case.ctx.variant_name.startswith("simt_row_per_thread")
+
+
+@pytest.mark.parametrize("model,N", [(W.ACOUSTIC, 2), (W.ELASTIC, 2)])
+def test_row_per_thread_vs_node_per_thread_every_element(dg, model, N):
+    """Two LSRK steps on K = 162 000 elements, row-per-thread kernel against the fused node-per-thread kernel, every value."""
+    w = W.config(4, N=N, model=model, n=30)
+    w.ic = "random"
+    out = []
+    for opts in ({}, {"variant": 1, "elems_per_thread": 1}):
+        ctx = dg.from_workload(w, device=0, **opts)
+        if not out:
+            q32 = w.initial_fields(ctx.node_coords()).astype(np.float32)
+            dt = float(np.float32(ctx.stable_dt(0.5)))
+        d = torch.from_numpy(q32).cuda()
+        ctx.run(d.data_ptr(), dt, 2)
+        torch.cuda.synchronize()
+        out.append((ctx.variant_name, d))
+        ctx.close()
+    assert out[0][0].startswith("simt_row_per_thread") and out[1][0].startswith("simt_fused")
     err = float((out[0][1] - out[1][1]).double().norm() / out[1][1].double().norm())
     assert err <= 1e-5, (out[0][0], out[1][0], err)
 
