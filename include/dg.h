@@ -125,6 +125,27 @@ int dg_rhs(dg_ctx *ctx, const float *d_q, float *d_rhs, void *cuda_stream);
 int dg_step(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);
 /* nsteps LSRK steps in place on d_q (5*nsteps fused stage kernels, one copy if that is odd)     */
 int dg_run(dg_ctx *ctx, float *d_q, float dt, int nsteps, void *cuda_stream);
+/* dg_step for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same LSRK(5,4) step (row a7 of the path fused into the five stage kernels, BASELINE.json north_star),
+ * the same kernels, the same result as dg_step bit for bit -- but the work memory of the step (the residual, the
+ * ping-pong copy of q and, where the tensor-core kernel keeps padded rows, the private padded state) lives in ONE
+ * file-scope `static __device__` array of DG_STATIC_SCRATCH_BYTES inside the library instead of buffers owned by the
+ * context.  The call performs no cudaMalloc / cudaFree and calls no allocating library routine: it enqueues one memset
+ * of the part of the array it uses, the five stage kernels (plus two row re-pitch kernels for padded rows) and one
+ * device copy on `cuda_stream`.  (dg_create, at set-up, does allocate the context's constants; it also resolves the
+ * array's device address, once per device.)
+ *   d_q     DEVICE, [K][Nfields][Np] float, 16-byte aligned, updated in place; caller-owned.
+ *   limit   2 (3 with padded rows: tensor-core kernel at N = 4, 8, 10) arrays of K Nfields Np floats, each rounded up to
+ *           256 bytes, must fit in DG_STATIC_SCRATCH_BYTES; beyond that the call returns DG_ERR_ARG with a message that
+ *           names the size needed and the limit, and enqueues nothing.
+ *   sharing every context, every stream and every call on a device shares the one array, and it keeps the last call's
+ *           contents: each call clears what it uses first, so results never depend on earlier calls, but two calls that
+ *           overlap on the GPU (different streams, or different host threads without ordering) RACE on it -- order
+ *           them on one stream or with events.  The context's own residual (dg_stage, dg_run) is not touched.
+ *   cost    every GPU on which the library's module is loaded holds the DG_STATIC_SCRATCH_BYTES until the process exits.
+ * Errors: as dg_step; DG_ERR_CUDA if the array's address could not be resolved (cudaGetSymbolAddress).             */
+#define DG_STATIC_SCRATCH_BYTES (32 * 1024 * 1024)
+int dg_step_static(dg_ctx *ctx, float *d_q, float dt, void *cuda_stream);
 /* ONE low-storage stage with explicit coefficients, out of place (the building block of dg_run, exposed for
  * per-stage control: sampled full-size parity checks, multi-rate drivers):
  *   res <- a res + dt r(q_in);  q_out <- q_in + b res     (res is the context's residual array; a = 0 ignores it).

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <array>
 #include <new>
 #include <stdexcept>
@@ -167,6 +168,12 @@ struct dg_ctx {
   std::string variant;
 };
 
+// ---- work memory of dg_step_static (include/dg.h): a file-scope device array instead of cudaMalloc'ed buffers, for callers
+// that must not allocate.  Every GPU that loads the library holds these DG_STATIC_SCRATCH_BYTES until the process exits.
+// In host code the name is only a stand-in: the device address comes from cudaGetSymbolAddress (static_scratch_setup),
+// once per device, with that device current.
+static __device__ __align__(256) unsigned char dg_static_scratch[DG_STATIC_SCRATCH_BYTES];
+
 namespace {
 
 // Every device entry point runs on the context's device and leaves the caller's current device as it found it.
@@ -182,6 +189,27 @@ struct DeviceGuard {
     if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
   }
 };
+constexpr int STATIC_SCRATCH_MAX_DEVICES = 64;
+std::mutex g_scratch_mu;
+unsigned char *g_scratch_ptr[STATIC_SCRATCH_MAX_DEVICES];      // device address of dg_static_scratch, per device
+int g_scratch_state[STATIC_SCRATCH_MAX_DEVICES];               // 0 = not asked yet, 1 = resolved, else -(cudaError_t)
+// Resolves the device address of dg_static_scratch on device `dev`, which must be current (dg_create and dg_step_static hold
+// a DeviceGuard).  Called at set-up by dg_create; never fatal there: a failure is kept and reported by dg_step_static.
+void static_scratch_setup(int dev) {
+  if (dev < 0 || dev >= STATIC_SCRATCH_MAX_DEVICES) return;
+  std::lock_guard<std::mutex> lock(g_scratch_mu);
+  if (g_scratch_state[dev] == 1) return;
+  void *ptr = nullptr;
+  const cudaError_t e = cudaGetSymbolAddress(&ptr, dg_static_scratch);
+  if (e == cudaSuccess && ptr) {
+    g_scratch_ptr[dev] = static_cast<unsigned char *>(ptr);
+    g_scratch_state[dev] = 1;
+  } else {
+    g_scratch_state[dev] = e == cudaSuccess ? -(int)cudaErrorInvalidSymbol : -(int)e;
+    (void)cudaGetLastError();
+  }
+}
+
 template <class T>
 T *upload(const std::vector<T> &h) {
   T *d = nullptr;
@@ -578,6 +606,7 @@ int dg_create(dg_ctx **out, const dg_mesh *mesh, int N, int model, const dg_mate
     if (c->device >= 0) {
       DeviceGuard guard(c->device);              // dg_create leaves the caller's current device unchanged
       if (!guard.ok) throw std::runtime_error("cuda: cannot select device " + std::to_string(c->device));
+      static_scratch_setup(c->device);           // (address of the static work memory of dg_step_static; allocates nothing)
       const int Np = c->Np, Nfp = c->Nfp;
       std::vector<float> DT((size_t)3 * Np * Np), LT((size_t)4 * Nfp * Np);
       const std::vector<double> *Dm[3] = {&c->ref.Dr, &c->ref.Ds, &c->ref.Dt};
@@ -860,6 +889,58 @@ int dg_run(dg_ctx *c, float *d_q, float dt, int nsteps, void *stream) {
 }
 
 int dg_step(dg_ctx *c, float *d_q, float dt, void *stream) { return dg_run(c, d_q, dt, 1, stream); }
+
+// One LSRK step like dg_step, with the residual and the ping-pong state (and, for the padded-row degrees of the tensor-core
+// kernel, the private padded copy of q) in dg_static_scratch instead of the context's buffers.  No cudaMalloc / cudaFree
+// and no allocating library call: memset, the stage kernels, the row re-pitch kernel and one device copy.
+int dg_step_static(dg_ctx *c, float *d_q, float dt, void *stream) {
+  DG_ENTER_DEVICE(c);
+  if (!d_q) return fail(DG_ERR_ARG, "NULL device pointer");
+  if (c->device >= STATIC_SCRATCH_MAX_DEVICES) return fail(DG_ERR_ARG, "dg_step_static: device ordinal beyond the address table");
+  static_scratch_setup(c->device);                // (normally a no-op: resolved by dg_create)
+  unsigned char *base = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_scratch_mu);
+    if (g_scratch_state[c->device] != 1)
+      return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString((cudaError_t)(-g_scratch_state[c->device])) +
+                                   " resolving the address of the static work memory (cudaGetSymbolAddress)");
+    base = g_scratch_ptr[c->device];
+  }
+  const bool pad = padded(c);
+  const size_t pitch = c->tc3 ? (size_t)c->PT : (size_t)c->Np;
+  const size_t arr = ((size_t)c->K * c->NF * pitch * sizeof(float) + 255) / 256 * 256;     // one array, 256-byte granules
+  const size_t narr = pad ? 3 : 2, need = narr * arr;
+  if (need > (size_t)DG_STATIC_SCRATCH_BYTES)
+    return fail(DG_ERR_ARG, "dg_step_static: this context needs " + std::to_string(need) + " bytes of work memory (" + std::to_string(narr) +
+                                " arrays of K Nf Np floats), the static array holds DG_STATIC_SCRATCH_BYTES = " +
+                                std::to_string((size_t)DG_STATIC_SCRATCH_BYTES) + ": use dg_step");
+  cudaStream_t st = (cudaStream_t)stream;
+  // the array keeps the last call's contents: everything this call uses starts from zero (the pad columns of padded rows
+  // must be zero, and stay zero; the residual is overwritten by stage 1, A_1 = 0)
+  cudaError_t e = cudaMemsetAsync(base, 0, need, st);
+  if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e) + " clearing the static work memory");
+  float *res = reinterpret_cast<float *>(base), *q2 = reinterpret_cast<float *>(base + arr);
+  float *qa = pad ? reinterpret_cast<float *>(base + 2 * arr) : d_q;
+  int launches = 1;
+  if (pad) {
+    if (int rc = copy_rows(c, qa, c->PT, d_q, c->Np, st)) return rc;
+    ++launches;
+  }
+  float *cur = qa, *oth = q2;
+  for (int i = 0; i < 5; ++i) {
+    if (int rc = launch_stage(c, c->k_stage, cur, oth, nullptr, (float)RK_A[i], (float)RK_B[i], dt, st, 0, -1, res)) return rc;
+    std::swap(cur, oth);
+    ++launches;
+  }
+  if (pad) {
+    if (int rc = copy_rows(c, d_q, c->Np, cur, c->PT, st)) return rc;
+  } else {
+    e = cudaMemcpyAsync(d_q, cur, (size_t)c->K * c->NF * c->Np * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return fail(DG_ERR_CUDA, std::string("cuda: ") + cudaGetErrorString(e));
+  }
+  c->last_launches = launches + 1 + c->iface_launches;
+  return DG_OK;
+}
 
 int dg_stage(dg_ctx *c, const float *d_q_in, float *d_q_out, float a, float b, float dt, void *stream) {
   DG_ENTER_DEVICE(c);

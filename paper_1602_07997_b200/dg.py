@@ -13,6 +13,7 @@ import numpy as np
 
 ACOUSTIC, ELASTIC = 0, 1
 BC_INTERIOR, BC_RIGID, BC_FREE, BC_SLIP = 0, 1, 2, 3
+STATIC_SCRATCH_BYTES = 32 * 1024 * 1024      # include/dg.h: DG_STATIC_SCRATCH_BYTES (work memory of dg_step_static)
 
 _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libdg.so")
 if not os.path.exists(_LIB_PATH):
@@ -35,7 +36,7 @@ class _Options(C.Structure):
 
 
 EXPORTS = ["dg_create", "dg_destroy", "dg_num_fields", "dg_np", "dg_nfp", "dg_num_elements", "dg_node_coords",
-           "dg_stable_dt", "dg_rhs", "dg_step", "dg_run", "dg_stage", "dg_stage_range", "dg_range_alignment", "dg_element_dt", "dg_ab3_step", "dg_ab3_run", "dg_ab3_reset", "dg_last_launch_count",
+           "dg_stable_dt", "dg_rhs", "dg_step", "dg_step_static", "dg_run", "dg_stage", "dg_stage_range", "dg_range_alignment", "dg_element_dt", "dg_ab3_step", "dg_ab3_run", "dg_ab3_reset", "dg_last_launch_count",
            "dg_variant_name", "dg_reference_operators", "dg_geometry", "dg_connectivity", "dg_last_error",
            "dg_partition_create", "dg_partition_destroy", "dg_partition_num_owned", "dg_partition_num_ghost",
            "dg_partition_global_ids", "dg_partition_local_mesh", "dg_partition_num_peers", "dg_partition_peer",
@@ -54,6 +55,7 @@ _lib.dg_stable_dt.argtypes = [C.c_void_p, C.c_double]
 _lib.dg_stable_dt.restype = C.c_double
 _lib.dg_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.dg_step.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
+_lib.dg_step_static.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_void_p]
 _lib.dg_run.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int, C.c_void_p]
 _lib.dg_stage.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
 _lib.dg_stage_range.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int64, C.c_int64, C.c_void_p]
@@ -192,6 +194,11 @@ class Context:
 
     def step(self, d_q: int, dt: float, stream: int | None = None):
         _check(_lib.dg_step(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))
+
+    def step_static(self, d_q: int, dt: float, stream: int | None = None):
+        """dg_step_static: the same step with its work memory in the library's static device array (no allocation;
+        limit STATIC_SCRATCH_BYTES; calls that overlap on the GPU race on the array: include/dg.h)."""
+        _check(_lib.dg_step_static(self._h, C.c_void_p(d_q), C.c_float(dt), C.c_void_p(stream or 0)))
 
     def run(self, d_q: int, dt: float, nsteps: int, stream: int | None = None):
         _check(_lib.dg_run(self._h, C.c_void_p(d_q), C.c_float(dt), int(nsteps), C.c_void_p(stream or 0)))
