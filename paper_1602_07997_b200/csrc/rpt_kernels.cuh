@@ -155,6 +155,9 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
   const float *g = sg + el * C::GP;
   const size_t base = ((size_t)k * NF + f) * NP;
 
+  // (Copying the whole element behind every face of the tile into shared memory with 16-byte cp.async and reading the traces
+  // from there -- 10 wide copies instead of 24 scattered 4-byte loads per tile at acoustic N = 2 -- was measured: 0.72 ->
+  // 0.96 ms per stage, elastic 1.89 -> 2.54: it moves 1.7x the bytes through L1 and costs a resident CTA per SM.)
   // ---- exterior traces of this lane's share of the element's face nodes (row a4): every load is issued here, without
   // a branch in between, so that the chain neighbour node -> values is in flight behind the volume term (a lane with no
   // task at t, or a boundary face, reads a valid address and ignores the value)
@@ -205,9 +208,12 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
     sp[i] = sq + (el * NF + src[i]) * NPP;
     mean[i] = __shfl_sync(0xffffffffu, mean_own, el * NF + src[i]);
   }
-  float r[NP];
+  // the row's accumulators as register pairs: an operator pair (n, n + 1) comes from the constant bank as one uniform
+  // 64-bit operand, and FFMA2 (the packed FP32 FMA of sm_100) does two nodes per issue slot: half the FMA instructions
+  static_assert(NP % 2 == 0, "row accumulators are paired");
+  float2 r2[NP / 2];
 #pragma unroll
-  for (int n = 0; n < NP; ++n) r[n] = 0.f;
+  for (int n = 0; n < NP / 2; ++n) r2[n] = make_float2(0.f, 0.f);
 #pragma unroll
   for (int m = 0; m < NP; ++m) {
     const float u0 = sp[0][m] - mean[0], u1 = sp[1][m] - mean[1], u2 = sp[2][m] - mean[2];
@@ -215,9 +221,12 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
 #pragma unroll
     for (int j = 0; j < 3; ++j) a[j] = cf[j][0] * u0 + cf[j][1] * u1 + cf[j][2] * u2;
 #pragma unroll
-    for (int j = 0; j < 3; ++j)
+    for (int j = 0; j < 3; ++j) {
+      const float2 aa = make_float2(a[j], a[j]);
 #pragma unroll
-      for (int n = 0; n < NP; ++n) r[n] = fmaf(c_rpt_D[(3 * m + j) * NP + n], a[j], r[n]);
+      for (int n = 0; n < NP / 2; ++n)
+        r2[n] = __ffma2_rn(make_float2(c_rpt_D[(3 * m + j) * NP + 2 * n], c_rpt_D[(3 * m + j) * NP + 2 * n + 1]), aa, r2[n]);
+    }
   }
 
   // ---- surface term (row a5): penalty terms of this lane's face nodes -> tile
@@ -280,11 +289,14 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
     const float *fr = sf + row * FP;
 #pragma unroll
     for (int j = 0; j < NFACE; ++j) {
-      const float Fj = fr[j];
+      const float2 Fj = make_float2(fr[j], fr[j]);
 #pragma unroll
-      for (int n = 0; n < NP; ++n) r[n] = fmaf(c_rpt_L[j * NP + n], Fj, r[n]);
+      for (int n = 0; n < NP / 2; ++n) r2[n] = __ffma2_rn(make_float2(c_rpt_L[j * NP + 2 * n], c_rpt_L[j * NP + 2 * n + 1]), Fj, r2[n]);
     }
   }
+  float r[NP];
+#pragma unroll
+  for (int n = 0; n < NP / 2; ++n) { r[2 * n] = r2[n].x; r[2 * n + 1] = r2[n].y; }
   // ---- LSRK update (row a7), rows as vectors of VW values
   if (valid) {
   auto ldv = [&](const float *ptr, int n, float (&x)[VW]) {
