@@ -182,6 +182,7 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
     for (int t = 0; t < TG; ++t) fetch(t, up[t]);
   }
   // the residual of this row (LSRK stage with A_s != 0): fetched here, used in the update
+  // (bringing the residual rows in with the tile through cp.async instead was measured: acoustic N = 2 0.685 -> 0.738 ms)
   constexpr bool RESPF = MODE == MODE_STAGE;
   float ores[RESPF ? NP : 1];
   if (RESPF && p.a != 0.f) {
@@ -297,36 +298,49 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
   float r[NP];
 #pragma unroll
   for (int n = 0; n < NP / 2; ++n) { r[2 * n] = r2[n].x; r[2 * n + 1] = r2[n].y; }
-  // ---- LSRK update (row a7), rows as vectors of VW values
-  if (valid) {
+  // ---- LSRK update (row a7).  Results leave through the tiles: a lane's row in global memory is Np floats at a stride of
+  // Np floats -- a vector store per lane touches one line per row, ten lines per instruction at N = 2 -- while the warp's
+  // rows together are one contiguous run.  So each lane writes its new q row over its (now unused) row of the field slot
+  // and its residual / right-hand side over its row of the penalty tile, and the warp copies both out line by line.
+  // (same-box A/B, ms per stage: acoustic N = 2 0.723 -> 0.684, N = 3 1.29 -> 1.08; the elastic tiles -- 27 rows -- and N = 1
+  // gain no lines and pay the extra shared-memory traffic: elastic N = 2 1.90 -> 1.97, acoustic N = 1 0.87 -> 0.93: direct there)
+  constexpr bool COUT = MODEL == 0 && N >= 2;
+  float *sqw = s_qt[w][slot] + row * NPP;                                // this lane's row of the field slot
+  float *sfw = sf + row * FP;                                            // and of the penalty tile
   auto ldv = [&](const float *ptr, int n, float (&x)[VW]) {
     const Vec v = *reinterpret_cast<const Vec *>(ptr + n);
     if constexpr (VW == 4) { x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w; }
     else if constexpr (VW == 2) { x[0] = v.x; x[1] = v.y; }
     else { x[0] = v; }
   };
-  auto stv = [&](float *ptr, int n, const float (&x)[VW]) {
-    Vec v;
-    if constexpr (VW == 4) v = make_float4(x[0], x[1], x[2], x[3]);
-    else if constexpr (VW == 2) v = make_float2(x[0], x[1]);
-    else v = x[0];
-    *reinterpret_cast<Vec *>(ptr + n) = v;
+  auto stv = [&](float *gptr, float *srow, int n, const float (&x)[VW]) {
+    if (COUT) {
+#pragma unroll
+      for (int t = 0; t < VW; ++t) srow[n + t] = x[t];
+    } else {
+      Vec v;
+      if constexpr (VW == 4) v = make_float4(x[0], x[1], x[2], x[3]);
+      else if constexpr (VW == 2) v = make_float2(x[0], x[1]);
+      else v = x[0];
+      *reinterpret_cast<Vec *>(gptr + n) = v;
+    }
   };
+  if (valid) {
 #pragma unroll
   for (int n = 0; n < NP; n += VW) {
     float rr[VW], qq[VW];
 #pragma unroll
     for (int t = 0; t < VW; ++t) { rr[t] = r[n + t]; qq[t] = own[n + t]; }
     if (MODE == MODE_RHS) {
-      stv(p.rhs + base, n, rr);
+      stv(p.rhs + base, sfw, n, rr);
     } else if (MODE == MODE_AB3) {
       float x[VW], y[VW];
       ldv(p.res + base, n, x);
       ldv(p.hist2 + base, n, y);
-      stv(p.rhs + base, n, rr);
+      stv(p.rhs + base, sfw, n, rr);
 #pragma unroll
       for (int t = 0; t < VW; ++t) qq[t] = fmaf(p.b, y[t], fmaf(p.a, x[t], fmaf(p.dt, rr[t], qq[t])));
-      stv(p.q_out + base, n, qq);
+      stv(p.q_out + base, sqw, n, qq);
     } else {
       float rs[VW];
 #pragma unroll
@@ -342,12 +356,28 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
 #pragma unroll
         for (int t = 0; t < VW; ++t) rs[t] = fmaf(p.a, o[t], rs[t]);
       }
-      stv(p.res + base, n, rs);
+      stv(p.res + base, sfw, n, rs);
 #pragma unroll
       for (int t = 0; t < VW; ++t) qq[t] = fmaf(p.b, rs[t], qq[t]);
-      stv(p.q_out + base, n, qq);
+      stv(p.q_out + base, sqw, n, qq);
     }
   }
+  }
+  if (COUT) {
+    __syncwarp();
+    const int total = nel * NF * NP;
+    const size_t g0 = (size_t)ke0 * NF * NP;
+    float *gr = (MODE == MODE_STAGE ? p.res : p.rhs) + g0;               // what the penalty tile carries
+    const float *sqt = s_qt[w][slot];
+#pragma unroll
+    for (int i = 0; i < (EPW * NF * NP + 31) / 32; ++i) {
+      const int idx = i * 32 + lane;
+      if (idx < total) {
+        const int rw = idx / NP;
+        gr[idx] = sf[idx + rw * (FP - NP)];
+        if (MODE != MODE_RHS) p.q_out[g0 + idx] = sqt[idx + rw * (NPP - NP)];
+      }
+    }
   }
   __syncwarp();                                                          // (every lane is done with this slot and the penalty tile)
   }
