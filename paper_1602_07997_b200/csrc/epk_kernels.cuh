@@ -18,6 +18,20 @@
 #include "flux.cuh"
 #include "kernels.cuh"
 
+// (development switches of the warp-cooperative staging paths below; the defaults are the measured best)
+#ifndef DG_X_EPK_GIN
+#define DG_X_EPK_GIN 1
+#endif
+#ifndef DG_X_EPK_QIN
+#define DG_X_EPK_QIN 0
+#endif
+#ifndef DG_X_EPK_GINE
+#define DG_X_EPK_GINE 0      // elastic N = 1 records through the tile: measured 1.62 -> 1.66 ms (it is bound by the trace gathers)
+#endif
+#ifndef DG_X_EPK_COUT
+#define DG_X_EPK_COUT 1
+#endif
+
 namespace dgk {
 
 constexpr int EPK_MAXNP = 10, EPK_MAXNFP = 6, EPK_MAXNFACE = 24;     // N <= 2
@@ -47,9 +61,16 @@ struct EpkFmask {
 
 // resident CTAs per SM asked of the compiler: the kernel is bound by the latency of its scattered gathers, so occupancy pays
 // as long as the register cap does not spill much (same-box A/B, ms per stage: acoustic N = 1 0.752 -> 0.713 with six CTAs;
-// elastic N = 1 1.772 -> 1.658 and acoustic N = 2 0.801 -> 0.789 with four; five or six CTAs there spill and lose 12-75 %)
+// elastic N = 1 1.772 -> 1.658 and acoustic N = 2 0.801 -> 0.789 with four; five or six CTAs there spill and lose 12-75 %).
+// With the records staged through shared memory (below) acoustic N = 1 is best at five: 0.603 (six, spills) -> 0.556.
 template <int MODEL, int N>
-constexpr int epk_min_ctas() { return (MODEL == 0 && N == 1) ? 6 : 4; }
+constexpr int epk_min_ctas() {
+#ifdef DG_X_EPK_MINB
+  return DG_X_EPK_MINB;
+#else
+  return (MODEL == 0 && N == 1) ? 5 : 4;
+#endif
+}
 
 template <int MODEL, int N, int MODE>
 __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kernel(const StageParams p) {
@@ -62,8 +83,10 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   // N = 1, acoustic: an element is four 16-byte vectors (one per field), and the four lanes of a quad gather their
   // neighbours' elements together (below): every lane stays alive, lanes beyond the range redo the last element and store nothing
   constexpr bool COOP = NP == 4 && MODEL == 0;
+  __shared__ float4 s_x[COOP ? 128 * 5 : 1];                          // per thread a padded row of five vectors (conflict-free)
   const int k_raw = p.kbeg + blockIdx.x * blockDim.x + threadIdx.x;
-  if (!COOP && k_raw >= p.K) return;
+  constexpr bool ALIVE = COOP || (MODEL == 1 && NP == 4 && DG_X_EPK_GINE);   // warp-cooperative staging: every lane stays
+  if (!ALIVE && k_raw >= p.K) return;
   const bool active = k_raw < p.K;
   const int k = active ? k_raw : p.K - 1;
 
@@ -72,14 +95,53 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   // the first 16 for the elastic one (its face records are read through L1 when needed: register pressure)
   constexpr int NGL = MODEL == 0 ? NGEO : 16;
   const float *g = p.geo + (size_t)k * NGEO;
+  // N = 1, acoustic: the warp's 32 geometric records (4 KB) and field rows (2 KB) are contiguous runs: the warp loads them
+  // four lines per instruction into padded shared-memory rows and every lane picks up its own (a 16-byte load per lane at
+  // a stride of 128 | 64 bytes touches 32 | 16 lines per instruction; the kernel is bound by exactly those L1 tag lookups)
+  constexpr bool GIN = (COOP && DG_X_EPK_GIN) || (MODEL == 1 && NP == 4 && DG_X_EPK_GINE), QIN = COOP && DG_X_EPK_QIN;
+  constexpr int GP4 = NGEO / 4 + 1;                                    // row pitch of the record tile, in vectors: odd
+  __shared__ float4 s_g[GIN ? 128 * GP4 : 1];
+  const int lane_ = threadIdx.x & 31, kw_ = k_raw - lane_, nvalid_ = min(32, p.K - kw_);
+  if (nvalid_ <= 0) return;                                            // (a warp wholly beyond the range)
   float gl[NGL];
+  if (GIN) {
+    float4 *gwarp = s_g + (threadIdx.x & ~31) * GP4;
+    const float4 *gsrc = reinterpret_cast<const float4 *>(p.geo) + (size_t)kw_ * (NGEO / 4);
 #pragma unroll
-  for (int i = 0; i < NGL / 4; ++i) {
-    const float4 v = __ldg(reinterpret_cast<const float4 *>(g) + i);
-    gl[4 * i] = v.x; gl[4 * i + 1] = v.y; gl[4 * i + 2] = v.z; gl[4 * i + 3] = v.w;
+    for (int it = 0; it < NGEO / 4; ++it) {
+      const int idx = it * 32 + lane_, e = idx / (NGEO / 4), v = idx - e * (NGEO / 4);
+      gwarp[e * GP4 + v] = __ldg(gsrc + (size_t)min(e, nvalid_ - 1) * (NGEO / 4) + v);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < NGL / 4; ++i) {
+      const float4 v = s_g[threadIdx.x * GP4 + i];
+      gl[4 * i] = v.x; gl[4 * i + 1] = v.y; gl[4 * i + 2] = v.z; gl[4 * i + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < NGL / 4; ++i) {
+      const float4 v = __ldg(reinterpret_cast<const float4 *>(g) + i);
+      gl[4 * i] = v.x; gl[4 * i + 1] = v.y; gl[4 * i + 2] = v.z; gl[4 * i + 3] = v.w;
+    }
   }
   float q[NV], r[NV];
-  {
+  if (QIN) {
+    float4 *xwarp = s_x + (threadIdx.x & ~31) * 5;
+    const float4 *qsrc = reinterpret_cast<const float4 *>(p.q_in) + (size_t)kw_ * (NV / 4);
+#pragma unroll
+    for (int it = 0; it < NV / 4; ++it) {
+      const int idx = it * 32 + lane_, e = idx / (NV / 4), v = idx - e * (NV / 4);
+      xwarp[e * 5 + v] = __ldg(qsrc + (size_t)min(e, nvalid_ - 1) * (NV / 4) + v);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < NV / 4; ++i) {
+      const float4 v = s_x[threadIdx.x * 5 + i];
+      q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
+    }
+    __syncwarp();                                                      // (the rows are reused by the face gather)
+  } else {
     const float4 *src = reinterpret_cast<const float4 *>(p.q_in + (size_t)k * NV);
 #pragma unroll
     for (int i = 0; i < NV / 4; ++i) {
@@ -183,8 +245,13 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   for (int f = 0; f < 4; ++f) {
     constexpr int FO = MODEL == 0 ? 12 : 16, FS = MODEL == 0 ? 5 : 8;
     float fg[8];
+    if (MODEL == 1 && GIN) {                                             // elastic: the face record from this thread's row of the tile
+      const float4 a = s_g[threadIdx.x * GP4 + (GIN ? (FO + FS * f) / 4 : 0)], b = s_g[threadIdx.x * GP4 + (GIN ? (FO + FS * f) / 4 + 1 : 0)];
+      fg[0] = a.x; fg[1] = a.y; fg[2] = a.z; fg[3] = a.w; fg[4] = b.x; fg[5] = b.y; fg[6] = b.z; fg[7] = b.w;
+    } else {
 #pragma unroll
-    for (int i = 0; i < FS; ++i) fg[i] = MODEL == 0 ? gl[(FO + FS * f + i) % NGL] : __ldg(g + FO + FS * f + i);
+      for (int i = 0; i < FS; ++i) fg[i] = MODEL == 0 ? gl[(FO + FS * f + i) % NGL] : __ldg(g + FO + FS * f + i);
+    }
     const float nx = fg[0], ny = fg[1], nz = fg[2];
     const int nb = f == 0 ? nbr4.x : (f == 1 ? nbr4.y : (f == 2 ? nbr4.z : nbr4.w));      // (f is a compile-time constant: unrolled)
     const int code = (int)((code4 >> (8 * f)) & 255u);
@@ -197,7 +264,6 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
       // instruction).  Lane j of a quad loads vector j (= field j) of the neighbour of each of the quad's four elements in
       // turn -- 8 lines per warp instruction instead of 32 -- and the quad transposes the 4 x 4 vectors through a padded
       // shared-memory row per lane (conflict-free 16-byte accesses).
-      __shared__ float4 s_x[128 * 5];
       const int lane = threadIdx.x & 31, qj = lane & 3, qb = lane & ~3;
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
@@ -276,6 +342,70 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   }
 
   // ---- LSRK update (row a7), 16-byte vectors
+  if (COOP && DG_X_EPK_COUT) {
+    // N = 1, acoustic: a thread's element is a 64-byte run, so a vector store per lane touches 16 lines per warp instruction.
+    // Results leave through the padded shared-memory rows instead, and the warp writes its 32 elements -- one contiguous
+    // 2 KB run -- four lines per instruction.
+    const int lane = threadIdx.x & 31;
+    const int kw = k_raw - lane, nvalid = min(32, p.K - kw);
+    float4 *srow = s_x + threadIdx.x * 5, *swarp = s_x + (threadIdx.x & ~31) * 5;
+    auto put = [&](const float *x) {
+#pragma unroll
+      for (int i = 0; i < NV / 4; ++i) srow[i] = make_float4(x[4 * i], x[4 * i + 1], x[4 * i + 2], x[4 * i + 3]);
+    };
+    auto out = [&](float *gdst) {
+      __syncwarp();
+      float4 *dst = reinterpret_cast<float4 *>(gdst + (size_t)kw * NV);
+#pragma unroll
+      for (int it = 0; it < NV / 4; ++it) {
+        const int idx = it * 32 + lane, e = idx / (NV / 4), v = idx - e * (NV / 4);
+        if (e < nvalid) dst[idx] = swarp[e * 5 + v];
+      }
+      __syncwarp();
+    };
+    const size_t base = (size_t)k * NV;
+    if (MODE == MODE_RHS) {
+      put(r);
+      out(p.rhs);
+    } else if (MODE == MODE_AB3) {
+      const float4 *h1 = reinterpret_cast<const float4 *>(p.res + base), *h2 = reinterpret_cast<const float4 *>(p.hist2 + base);
+#pragma unroll
+      for (int i = 0; i < NV / 4; ++i) {
+        const float4 x = h1[i], y = __ldg(h2 + i);
+        q[4 * i] = fmaf(p.b, y.x, fmaf(p.a, x.x, fmaf(p.dt, r[4 * i], q[4 * i])));
+        q[4 * i + 1] = fmaf(p.b, y.y, fmaf(p.a, x.y, fmaf(p.dt, r[4 * i + 1], q[4 * i + 1])));
+        q[4 * i + 2] = fmaf(p.b, y.z, fmaf(p.a, x.z, fmaf(p.dt, r[4 * i + 2], q[4 * i + 2])));
+        q[4 * i + 3] = fmaf(p.b, y.w, fmaf(p.a, x.w, fmaf(p.dt, r[4 * i + 3], q[4 * i + 3])));
+      }
+      __syncwarp();                                                    // (every lane has read its history rows: p.rhs may alias none of them, but keep order)
+      put(r);
+      out(p.rhs);
+      put(q);
+      out(p.q_out);
+    } else {
+      const float4 *pres = reinterpret_cast<const float4 *>(p.res + base);
+#pragma unroll
+      for (int i = 0; i < NV / 4; ++i) {
+        float rs[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) rs[t] = p.dt * r[4 * i + t];
+        if (p.a != 0.f) {
+          const float4 o = pres[i];
+          rs[0] = fmaf(p.a, o.x, rs[0]); rs[1] = fmaf(p.a, o.y, rs[1]); rs[2] = fmaf(p.a, o.z, rs[2]); rs[3] = fmaf(p.a, o.w, rs[3]);
+        }
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          r[4 * i + t] = rs[t];
+          q[4 * i + t] = fmaf(p.b, rs[t], q[4 * i + t]);
+        }
+      }
+      put(r);
+      out(p.res);
+      put(q);
+      out(p.q_out);
+    }
+    return;
+  }
   if (!active) return;                                                 // (lanes kept alive for the quad gather only)
   const size_t base = (size_t)k * NV;
   if (MODE == MODE_RHS) {
