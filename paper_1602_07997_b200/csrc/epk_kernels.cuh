@@ -31,6 +31,12 @@
 #ifndef DG_X_EPK_COUT
 #define DG_X_EPK_COUT 1
 #endif
+#ifndef DG_X_EPK_COUTE
+#define DG_X_EPK_COUTE 0     // elastic N = 1 results through the tile: 1.62 -> 1.60 ms per stage, dg_rhs 1.32 -> 1.37: left off
+#endif
+#ifndef DG_X_EPK_QINE
+#define DG_X_EPK_QINE 0      // elastic N = 1 fields through the tile: 1.60 -> 1.71 ms
+#endif
 
 namespace dgk {
 
@@ -83,9 +89,11 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   // N = 1, acoustic: an element is four 16-byte vectors (one per field), and the four lanes of a quad gather their
   // neighbours' elements together (below): every lane stays alive, lanes beyond the range redo the last element and store nothing
   constexpr bool COOP = NP == 4 && MODEL == 0;
-  __shared__ float4 s_x[COOP ? 128 * 5 : 1];                          // per thread a padded row of five vectors (conflict-free)
+  constexpr bool EL1 = MODEL == 1 && NP == 4;                          // elastic N = 1: nine vectors per element
+  constexpr int XP = (NV / 4) | 1;                                     // row pitch of the tile in vectors: odd (conflict-free)
+  __shared__ float4 s_x[(COOP || (EL1 && (DG_X_EPK_COUTE || DG_X_EPK_QINE))) ? 128 * XP : 1];   // per thread a padded row
   const int k_raw = p.kbeg + blockIdx.x * blockDim.x + threadIdx.x;
-  constexpr bool ALIVE = COOP || (MODEL == 1 && NP == 4 && DG_X_EPK_GINE);   // warp-cooperative staging: every lane stays
+  constexpr bool ALIVE = COOP || (MODEL == 1 && NP == 4 && (DG_X_EPK_GINE || DG_X_EPK_COUTE || DG_X_EPK_QINE));   // warp-cooperative staging: every lane stays
   if (!ALIVE && k_raw >= p.K) return;
   const bool active = k_raw < p.K;
   const int k = active ? k_raw : p.K - 1;
@@ -98,7 +106,7 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   // N = 1, acoustic: the warp's 32 geometric records (4 KB) and field rows (2 KB) are contiguous runs: the warp loads them
   // four lines per instruction into padded shared-memory rows and every lane picks up its own (a 16-byte load per lane at
   // a stride of 128 | 64 bytes touches 32 | 16 lines per instruction; the kernel is bound by exactly those L1 tag lookups)
-  constexpr bool GIN = (COOP && DG_X_EPK_GIN) || (MODEL == 1 && NP == 4 && DG_X_EPK_GINE), QIN = COOP && DG_X_EPK_QIN;
+  constexpr bool GIN = (COOP && DG_X_EPK_GIN) || (MODEL == 1 && NP == 4 && DG_X_EPK_GINE), QIN = (COOP && DG_X_EPK_QIN) || (EL1 && DG_X_EPK_QINE);
   constexpr int GP4 = NGEO / 4 + 1;                                    // row pitch of the record tile, in vectors: odd
   __shared__ float4 s_g[GIN ? 128 * GP4 : 1];
   const int lane_ = threadIdx.x & 31, kw_ = k_raw - lane_, nvalid_ = min(32, p.K - kw_);
@@ -127,17 +135,17 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   }
   float q[NV], r[NV];
   if (QIN) {
-    float4 *xwarp = s_x + (threadIdx.x & ~31) * 5;
+    float4 *xwarp = s_x + (threadIdx.x & ~31) * XP;
     const float4 *qsrc = reinterpret_cast<const float4 *>(p.q_in) + (size_t)kw_ * (NV / 4);
 #pragma unroll
     for (int it = 0; it < NV / 4; ++it) {
       const int idx = it * 32 + lane_, e = idx / (NV / 4), v = idx - e * (NV / 4);
-      xwarp[e * 5 + v] = __ldg(qsrc + (size_t)min(e, nvalid_ - 1) * (NV / 4) + v);
+      xwarp[e * XP + v] = __ldg(qsrc + (size_t)min(e, nvalid_ - 1) * (NV / 4) + v);
     }
     __syncwarp();
 #pragma unroll
     for (int i = 0; i < NV / 4; ++i) {
-      const float4 v = s_x[threadIdx.x * 5 + i];
+      const float4 v = s_x[threadIdx.x * XP + i];
       q[4 * i] = v.x; q[4 * i + 1] = v.y; q[4 * i + 2] = v.z; q[4 * i + 3] = v.w;
     }
     __syncwarp();                                                      // (the rows are reused by the face gather)
@@ -270,11 +278,11 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
         const int nbi = __shfl_sync(0xffffffffu, nb, qb + i);
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         if (nbi >= 0) v = __ldg(reinterpret_cast<const float4 *>(p.q_in + (size_t)nbi * NV) + qj);
-        s_x[((threadIdx.x & ~3) + i) * 5 + qj] = v;
+        s_x[((threadIdx.x & ~3) + i) * XP + qj] = v;
       }
       __syncwarp();
 #pragma unroll
-      for (int c = 0; c < NF; ++c) nq[c] = s_x[threadIdx.x * 5 + c];
+      for (int c = 0; c < NF; ++c) nq[c] = s_x[threadIdx.x * XP + c];
       __syncwarp();
     }
     auto pick = [](const float4 &v, int nn) { return (nn & 2) ? ((nn & 1) ? v.w : v.z) : ((nn & 1) ? v.y : v.x); };
@@ -342,13 +350,13 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   }
 
   // ---- LSRK update (row a7), 16-byte vectors
-  if (COOP && DG_X_EPK_COUT) {
+  if ((COOP && DG_X_EPK_COUT) || (EL1 && DG_X_EPK_COUTE)) {
     // N = 1, acoustic: a thread's element is a 64-byte run, so a vector store per lane touches 16 lines per warp instruction.
     // Results leave through the padded shared-memory rows instead, and the warp writes its 32 elements -- one contiguous
     // 2 KB run -- four lines per instruction.
     const int lane = threadIdx.x & 31;
     const int kw = k_raw - lane, nvalid = min(32, p.K - kw);
-    float4 *srow = s_x + threadIdx.x * 5, *swarp = s_x + (threadIdx.x & ~31) * 5;
+    float4 *srow = s_x + threadIdx.x * XP, *swarp = s_x + (threadIdx.x & ~31) * XP;
     auto put = [&](const float *x) {
 #pragma unroll
       for (int i = 0; i < NV / 4; ++i) srow[i] = make_float4(x[4 * i], x[4 * i + 1], x[4 * i + 2], x[4 * i + 3]);
@@ -359,7 +367,7 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
 #pragma unroll
       for (int it = 0; it < NV / 4; ++it) {
         const int idx = it * 32 + lane, e = idx / (NV / 4), v = idx - e * (NV / 4);
-        if (e < nvalid) dst[idx] = swarp[e * 5 + v];
+        if (e < nvalid) dst[idx] = swarp[e * XP + v];
       }
       __syncwarp();
     };
