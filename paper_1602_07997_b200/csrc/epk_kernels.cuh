@@ -26,16 +26,19 @@
 #define DG_X_EPK_QIN 0
 #endif
 #ifndef DG_X_EPK_GINE
-#define DG_X_EPK_GINE 0      // elastic N = 1 records through the tile: measured 1.62 -> 1.66 ms (it is bound by the trace gathers)
+#define DG_X_EPK_GINE 1      // elastic N = 1: records through the tile
 #endif
 #ifndef DG_X_EPK_COUT
 #define DG_X_EPK_COUT 1
 #endif
+#ifndef DG_X_EPK_VGE
+#define DG_X_EPK_VGE 1
+#endif
 #ifndef DG_X_EPK_COUTE
-#define DG_X_EPK_COUTE 0     // elastic N = 1 results through the tile: 1.62 -> 1.60 ms per stage, dg_rhs 1.32 -> 1.37: left off
+#define DG_X_EPK_COUTE 1     // elastic N = 1: results through the tile
 #endif
 #ifndef DG_X_EPK_QINE
-#define DG_X_EPK_QINE 0      // elastic N = 1 fields through the tile: 1.60 -> 1.71 ms
+#define DG_X_EPK_QINE 0      // elastic N = 1 fields through the tile: 1.27 -> 1.32 ms: off
 #endif
 
 namespace dgk {
@@ -69,12 +72,14 @@ struct EpkFmask {
 // as long as the register cap does not spill much (same-box A/B, ms per stage: acoustic N = 1 0.752 -> 0.713 with six CTAs;
 // elastic N = 1 1.772 -> 1.658 and acoustic N = 2 0.801 -> 0.789 with four; five or six CTAs there spill and lose 12-75 %).
 // With the records staged through shared memory (below) acoustic N = 1 is best at five: 0.603 (six, spills) -> 0.556.
+// Elastic N = 1 with whole-vector trace gathers (36 more live registers) wants three: 2.00 (four, 700 bytes of spills) -> 1.51;
+// with records and results through the tiles on top 1.27 (two CTAs 1.45, four 2.14).
 template <int MODEL, int N>
 constexpr int epk_min_ctas() {
 #ifdef DG_X_EPK_MINB
   return DG_X_EPK_MINB;
 #else
-  return (MODEL == 0 && N == 1) ? 5 : 4;
+  return N == 1 ? (MODEL == 0 ? 5 : 3) : 4;
 #endif
 }
 
@@ -265,9 +270,17 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
     const int code = (int)((code4 >> (8 * f)) & 255u);
     // N = 1: a field of the neighbour is one 16-byte vector (Np = 4): fetch it whole and pick the node afterwards
     // (a third of the gather instructions; the kernel is bound by the L1/LSU pipe, the ALUs are idle)
-    constexpr bool VGATHER = COOP;                               // (elastic N = 1: nine vectors per face cost more registers than they save)
+    // (elastic: nine vectors per face, this lane's own neighbour: a third of the load instructions and of the L1 wavefronts --
+    // ncu had 9 wavefronts per scalar gather request; same-box A/B 1.62 -> 1.51 ms per stage, dg_rhs 1.33 -> 1.09, at three CTAs per SM)
+    constexpr bool VGATHER = COOP || (MODEL == 1 && NP == 4 && DG_X_EPK_VGE);
     float4 nq[VGATHER ? NF : 1];
-    if (VGATHER && !p.pflux) {
+    if (VGATHER && !COOP && !p.pflux) {                                  // elastic N = 1: this lane's neighbour, nine whole vectors
+      if (nb >= 0) {
+#pragma unroll
+        for (int c = 0; c < NF; ++c) nq[c] = __ldg(reinterpret_cast<const float4 *>(p.q_in + (size_t)nb * NV) + c);
+      }
+    }
+    if (COOP && !p.pflux) {
       // Warp-level gather: the kernel is bound by the L1 tag stage (one 128-byte line per lane and load: 32 lines per warp
       // instruction).  Lane j of a quad loads vector j (= field j) of the neighbour of each of the quad's four elements in
       // turn -- 8 lines per warp instruction instead of 32 -- and the quad transposes the 4 x 4 vectors through a padded
