@@ -199,6 +199,12 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
   float cf[3][3];
   int src[3], nsrc;
   row_coefficients_s<MODEL>(g, f, cf, src, nsrc);
+  // the element's material constants in registers (the penalty terms below read them per face node; the stores to the
+  // penalty tile in between keep the compiler from holding shared-memory values across tasks)
+  float gm[14];
+#pragma unroll
+  for (int i = 9; i < 14; ++i) gm[i] = g[i];
+  const float *gpen = gm;                                               // (acoustic N = 2: 0.684 -> 0.673 ms per stage)
   const float *own = sq + row * NPP;
   // mean of the four vertex values of the row: D_j 1 = 0, so the shift is exact and removes the cancellation
   const float mean_own = 0.25f * ((own[0] + own[N]) + (own[NFP - 1] + own[NP - 1]));
@@ -262,7 +268,7 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
           } else {
             acoustic_boundary_jump(nb, um[0], um[1] * nx + um[2] * ny + um[3] * nz, dp, dvn);
           }
-          const float4 Pn = acoustic_penalty(g, fg, dp, dvn);
+          const float4 Pn = acoustic_penalty(gpen, fg, dp, dvn);
           F[0] = Pn.x; F[1] = Pn.y; F[2] = Pn.z; F[3] = Pn.w;
         } else {
           float Tmx, Tmy, Tmz;
@@ -276,7 +282,7 @@ __global__ void __launch_bounds__(Rpt<MODEL, N>::WARPS * 32, rpt_min_ctas<N>()) 
           } else {
             elastic_boundary_jump(nb, um, Tmx, Tmy, Tmz, nx, ny, nz, dv, dT);
           }
-          elastic_penalty(g, fg, dv, dT, F);
+          elastic_penalty(gpen, fg, dv, dT, F);
         }
       }
 #pragma unroll
