@@ -281,7 +281,7 @@ def test_row_per_thread_vs_node_per_thread_every_element(dg, model, N):
 # ---------------------------------------------------------------- multi-rate hook: a stage restricted to an element range
 @pytest.mark.parametrize("model,N,opts", [(W.ACOUSTIC, 1, {}), (W.ACOUSTIC, 3, {}), (W.ELASTIC, 3, {}), (W.ELASTIC, 5, {"max_ctas": 2}),
                                           (W.ELASTIC, 9, {}), (W.ACOUSTIC, 4, {"variant": 1}), (W.ELASTIC, 2, {"variant": 1}),
-                                          (W.ACOUSTIC, 3, {"variant": 5}), (W.ELASTIC, 2, {"variant": 5})])
+                                          (W.ACOUSTIC, 3, {"variant": 5}), (W.ELASTIC, 2, {"variant": 5}), (W.ELASTIC, 1, {}), (W.ACOUSTIC, 2, {"variant": 1})])
 def test_stage_range_composes_to_the_full_stage(dg, model, N, opts):
     """dg_stage_range over [0, k1), [k1, k2), [k2, K) -- the per-level launches of a multi-rate driver
     -- writes exactly what one dg_stage over the mesh writes, touches nothing outside its range (q_out and the residual),
