@@ -397,7 +397,12 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
           uint32_t vm[LW], vs[LW];
           T3_TIMED(2, tc::tmem_ld<LW>(t0 + LW * h, vm); tc::tmem_ld<LW>(t0 + NCH + LW * h, vs));
 #pragma unroll
-          for (int j = 0; j < LW; ++j) acc[LW * h + j] = __uint_as_float(vm[j]) + __uint_as_float(vs[j]);
+          for (int j = 0; j < LW; j += 2) {
+            const float2 sum = __fadd2_rn(make_float2(__uint_as_float(vm[j]), __uint_as_float(vm[j + 1])),
+                                          make_float2(__uint_as_float(vs[j]), __uint_as_float(vs[j + 1])));
+            acc[LW * h + j] = sum.x;
+            acc[LW * h + j + 1] = sum.y;
+          }
         }
       }
       if (c0 + CW >= ncv) {              // accumulators drained: the MMA warp may start the next batch on this set
@@ -426,14 +431,16 @@ __global__ void __launch_bounds__(T3_THREADS, 1) tc3_stage_kernel(const __grid_c
           *pr = make_float4(r[0], r[1], r[2], r[3]);
           *pq = make_float4(fmaf(p.b, H2.x, fmaf(p.a, H1.x, fmaf(p.dt, r[0], Q.x))), fmaf(p.b, H2.y, fmaf(p.a, H1.y, fmaf(p.dt, r[1], Q.y))),
                             fmaf(p.b, H2.z, fmaf(p.a, H1.z, fmaf(p.dt, r[2], Q.z))), fmaf(p.b, H2.w, fmaf(p.a, H1.w, fmaf(p.dt, r[3], Q.w))));
-        } else {
+        } else {                         // res <- a res + dt r; q <- q + b res, two values per instruction (FMUL2 / FFMA2)
           float4 R = make_float4(0.f, 0.f, 0.f, 0.f);
           if (need_res) R = *pr;
           const float4 Q = *pq;
-          R.x = fmaf(p.a, R.x, p.dt * r[0]); R.y = fmaf(p.a, R.y, p.dt * r[1]);
-          R.z = fmaf(p.a, R.z, p.dt * r[2]); R.w = fmaf(p.a, R.w, p.dt * r[3]);
-          *pr = R;
-          *pq = make_float4(fmaf(p.b, R.x, Q.x), fmaf(p.b, R.y, Q.y), fmaf(p.b, R.z, Q.z), fmaf(p.b, R.w, Q.w));
+          const float2 a2 = make_float2(p.a, p.a), b2 = make_float2(p.b, p.b), dt2 = make_float2(p.dt, p.dt);
+          const float2 R0 = __ffma2_rn(a2, make_float2(R.x, R.y), __fmul2_rn(dt2, make_float2(r[0], r[1])));
+          const float2 R1 = __ffma2_rn(a2, make_float2(R.z, R.w), __fmul2_rn(dt2, make_float2(r[2], r[3])));
+          const float2 Q0 = __ffma2_rn(b2, R0, make_float2(Q.x, Q.y)), Q1 = __ffma2_rn(b2, R1, make_float2(Q.z, Q.w));
+          *pr = make_float4(R0.x, R0.y, R1.x, R1.y);
+          *pq = make_float4(Q0.x, Q0.y, Q1.x, Q1.y);
         }
       }
       tc::fence_proxy_async();           // generic-proxy writes -> visible to the TMA store
