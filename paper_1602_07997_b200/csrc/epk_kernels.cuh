@@ -28,6 +28,9 @@
 #ifndef DG_X_EPK_GINE
 #define DG_X_EPK_GINE 1      // elastic N = 1: records through the tile
 #endif
+#ifndef DG_X_EPK_F2
+#define DG_X_EPK_F2 1          // volume and lift FMAs as FFMA2 on node pairs
+#endif
 #ifndef DG_X_EPK_COUT
 #define DG_X_EPK_COUT 1
 #endif
@@ -46,6 +49,9 @@ namespace dgk {
 constexpr int EPK_MAXNP = 10, EPK_MAXNFP = 6, EPK_MAXNFACE = 24;     // N <= 2
 static __constant__ float c_epk_D[3 * EPK_MAXNP * EPK_MAXNP];          // D_j[n][m] at (j Np + n) Np + m
 static __constant__ float c_epk_L[EPK_MAXNP * EPK_MAXNFACE];           // LIFT[n][j] at n 4Nfp + j
+// the same operators with the output node n fastest, so that a pair (n, n + 1) is one 64-bit constant-bank operand of FFMA2
+static __constant__ float c_epk_Dt[3 * EPK_MAXNP * EPK_MAXNP];         // D_j[n][m] at (j Np + m) Np + n
+static __constant__ float c_epk_Lt[EPK_MAXNFACE * EPK_MAXNP];          // LIFT[n][j] at j Np + n
 static __constant__ unsigned short c_epk_nbrnode[4 * 24 * EPK_MAXNFP]; // neighbour's volume node at (f 24 + code) Nfp + i
 
 // face masks in the library's order (host_setup.cpp: nodes in lattice order, t slowest, r fastest; a face lists its
@@ -91,6 +97,7 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
   constexpr int NV = NF * NP;                                          // values per element
   static_assert(NV % 4 == 0, "an element's fields are moved as 16-byte vectors");
   constexpr EpkFmask<N> FM{};
+  constexpr bool F2 = DG_X_EPK_F2 && NP == 4;                          // (N = 2: the pairs cost registers the kernel does not have: 356 bytes of spills)
   // N = 1, acoustic: an element is four 16-byte vectors (one per field), and the four lanes of a quad gather their
   // neighbours' elements together (below): every lane stays alive, lanes beyond the range redo the last element and store nothing
   constexpr bool COOP = NP == 4 && MODEL == 0;
@@ -183,22 +190,46 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
     }
     const float kap = gl[9], irho = gl[10];
 #pragma unroll
-    for (int n = 0; n < NP; ++n) {
-      float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+    for (int n = 0; n < NP; n += 2) {
+      // two output nodes per FFMA2 (the packed FP32 FMA of sm_100): the operator pair (n, n + 1) is one 64-bit constant operand
+      float2 A0 = make_float2(0.f, 0.f), A1 = A0, A2 = A0, A3 = A0;
+      float a0[2] = {0.f, 0.f}, a1[2] = {0.f, 0.f}, a2[2] = {0.f, 0.f}, a3[2] = {0.f, 0.f};
 #pragma unroll
       for (int m = 0; m < NP; ++m) {
-        const float dr = c_epk_D[(0 * NP + n) * NP + m], ds = c_epk_D[(1 * NP + n) * NP + m], dt = c_epk_D[(2 * NP + n) * NP + m];
-        a0 = fmaf(dr, u[m], a0);
-        a1 = fmaf(ds, u[m], a1);
-        a2 = fmaf(dt, u[m], a2);
-        a3 = fmaf(dr, w[0][m], a3);
-        a3 = fmaf(ds, w[1][m], a3);
-        a3 = fmaf(dt, w[2][m], a3);
+        if (F2) {
+          const float2 DR = make_float2(c_epk_Dt[(0 * NP + m) * NP + n], c_epk_Dt[(0 * NP + m) * NP + n + 1]);
+          const float2 DS = make_float2(c_epk_Dt[(1 * NP + m) * NP + n], c_epk_Dt[(1 * NP + m) * NP + n + 1]);
+          const float2 DT = make_float2(c_epk_Dt[(2 * NP + m) * NP + n], c_epk_Dt[(2 * NP + m) * NP + n + 1]);
+          const float2 um = make_float2(u[m], u[m]);
+          A0 = __ffma2_rn(DR, um, A0);
+          A1 = __ffma2_rn(DS, um, A1);
+          A2 = __ffma2_rn(DT, um, A2);
+          A3 = __ffma2_rn(DR, make_float2(w[0][m], w[0][m]), A3);
+          A3 = __ffma2_rn(DS, make_float2(w[1][m], w[1][m]), A3);
+          A3 = __ffma2_rn(DT, make_float2(w[2][m], w[2][m]), A3);
+        } else {
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const float dr = c_epk_D[(0 * NP + n + h) * NP + m], ds = c_epk_D[(1 * NP + n + h) * NP + m], dt = c_epk_D[(2 * NP + n + h) * NP + m];
+            a0[h] = fmaf(dr, u[m], a0[h]);
+            a1[h] = fmaf(ds, u[m], a1[h]);
+            a2[h] = fmaf(dt, u[m], a2[h]);
+            a3[h] = fmaf(dr, w[0][m], a3[h]);
+            a3[h] = fmaf(ds, w[1][m], a3[h]);
+            a3[h] = fmaf(dt, w[2][m], a3[h]);
+          }
+        }
+      }
+      if (F2) {
+        a0[0] = A0.x; a0[1] = A0.y; a1[0] = A1.x; a1[1] = A1.y; a2[0] = A2.x; a2[1] = A2.y; a3[0] = A3.x; a3[1] = A3.y;
       }
       // eq. (5)-(6)
-      r[n] = -kap * a3;
 #pragma unroll
-      for (int i = 0; i < 3; ++i) r[(1 + i) * NP + n] = -irho * (gl[3 * i] * a0 + gl[3 * i + 1] * a1 + gl[3 * i + 2] * a2);
+      for (int h = 0; h < 2; ++h) {
+        r[n + h] = -kap * a3[h];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) r[(1 + i) * NP + n + h] = -irho * (gl[3 * i] * a0[h] + gl[3 * i + 1] * a1[h] + gl[3 * i + 2] * a2[h]);
+      }
     }
   } else {
     // w_{i,n} = sum_m g_mn sigma_im ; fields vx vy vz sxx syy szz sxy sxz syz
@@ -215,23 +246,51 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
         w[i][2][m] = gl[2] * s0 + gl[5] * s1 + gl[8] * s2;
       }
 #pragma unroll
-    for (int n = 0; n < NP; ++n) {
-      float acc[12];
+    for (int n2 = 0; n2 < NP; n2 += 2) {
+      float2 ACC[12];
 #pragma unroll
-      for (int c = 0; c < 12; ++c) acc[c] = 0.f;
+      for (int c = 0; c < 12; ++c) ACC[c] = make_float2(0.f, 0.f);
+      float accs[2][12];
+#pragma unroll
+      for (int c = 0; c < 12; ++c) accs[0][c] = accs[1][c] = 0.f;
 #pragma unroll
       for (int m = 0; m < NP; ++m) {
-        const float dr = c_epk_D[(0 * NP + n) * NP + m], ds = c_epk_D[(1 * NP + n) * NP + m], dt = c_epk_D[(2 * NP + n) * NP + m];
+        if (F2) {
+          const float2 DR = make_float2(c_epk_Dt[(0 * NP + m) * NP + n2], c_epk_Dt[(0 * NP + m) * NP + n2 + 1]);
+          const float2 DS = make_float2(c_epk_Dt[(1 * NP + m) * NP + n2], c_epk_Dt[(1 * NP + m) * NP + n2 + 1]);
+          const float2 DT = make_float2(c_epk_Dt[(2 * NP + m) * NP + n2], c_epk_Dt[(2 * NP + m) * NP + n2 + 1]);
 #pragma unroll
-        for (int i = 0; i < 3; ++i) {
-          acc[3 * i + 0] = fmaf(dr, u[i * NP + m], acc[3 * i + 0]);
-          acc[3 * i + 1] = fmaf(ds, u[i * NP + m], acc[3 * i + 1]);
-          acc[3 * i + 2] = fmaf(dt, u[i * NP + m], acc[3 * i + 2]);
-          acc[9 + i] = fmaf(dr, w[i][0][m], acc[9 + i]);
-          acc[9 + i] = fmaf(ds, w[i][1][m], acc[9 + i]);
-          acc[9 + i] = fmaf(dt, w[i][2][m], acc[9 + i]);
+          for (int i = 0; i < 3; ++i) {
+            const float2 ui = make_float2(u[i * NP + m], u[i * NP + m]);
+            ACC[3 * i + 0] = __ffma2_rn(DR, ui, ACC[3 * i + 0]);
+            ACC[3 * i + 1] = __ffma2_rn(DS, ui, ACC[3 * i + 1]);
+            ACC[3 * i + 2] = __ffma2_rn(DT, ui, ACC[3 * i + 2]);
+            ACC[9 + i] = __ffma2_rn(DR, make_float2(w[i][0][m], w[i][0][m]), ACC[9 + i]);
+            ACC[9 + i] = __ffma2_rn(DS, make_float2(w[i][1][m], w[i][1][m]), ACC[9 + i]);
+            ACC[9 + i] = __ffma2_rn(DT, make_float2(w[i][2][m], w[i][2][m]), ACC[9 + i]);
+          }
+        } else {
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const float dr = c_epk_D[(0 * NP + n2 + h) * NP + m], ds = c_epk_D[(1 * NP + n2 + h) * NP + m], dt = c_epk_D[(2 * NP + n2 + h) * NP + m];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+              accs[h][3 * i + 0] = fmaf(dr, u[i * NP + m], accs[h][3 * i + 0]);
+              accs[h][3 * i + 1] = fmaf(ds, u[i * NP + m], accs[h][3 * i + 1]);
+              accs[h][3 * i + 2] = fmaf(dt, u[i * NP + m], accs[h][3 * i + 2]);
+              accs[h][9 + i] = fmaf(dr, w[i][0][m], accs[h][9 + i]);
+              accs[h][9 + i] = fmaf(ds, w[i][1][m], accs[h][9 + i]);
+              accs[h][9 + i] = fmaf(dt, w[i][2][m], accs[h][9 + i]);
+            }
+          }
         }
       }
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+      const int n = n2 + h;
+      float acc[12];
+#pragma unroll
+      for (int c = 0; c < 12; ++c) acc[c] = F2 ? (h == 0 ? ACC[c].x : ACC[c].y) : accs[h][c];
       float gv[3][3];   // gv[i][j] = d_j v_i = sum_m g_jm (D_m v_i)
 #pragma unroll
       for (int i = 0; i < 3; ++i)
@@ -247,6 +306,7 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
       r[6 * NP + n] = mu * (gv[0][1] + gv[1][0]);
       r[7 * NP + n] = mu * (gv[0][2] + gv[2][0]);
       r[8 * NP + n] = mu * (gv[1][2] + gv[2][1]);
+      }
     }
   }
 
@@ -353,11 +413,24 @@ __global__ void __launch_bounds__(128, epk_min_ctas<MODEL, N>()) epk_stage_kerne
         }
         elastic_penalty(gl, fg, dv, dT, F);
       }
+      if (F2) {
 #pragma unroll
-      for (int n = 0; n < NP; ++n) {
-        const float l = c_epk_L[n * NFACE + j];
+        for (int n = 0; n < NP; n += 2) {
+          const float2 l2 = make_float2(c_epk_Lt[j * NP + n], c_epk_Lt[j * NP + n + 1]);
 #pragma unroll
-        for (int c = 0; c < NF; ++c) r[c * NP + n] = fmaf(l, F[c], r[c * NP + n]);
+          for (int c = 0; c < NF; ++c) {
+            const float2 rp = __ffma2_rn(l2, make_float2(F[c], F[c]), make_float2(r[c * NP + n], r[c * NP + n + 1]));
+            r[c * NP + n] = rp.x;
+            r[c * NP + n + 1] = rp.y;
+          }
+        }
+      } else {
+#pragma unroll
+        for (int n = 0; n < NP; ++n) {
+          const float l = c_epk_L[n * NFACE + j];
+#pragma unroll
+          for (int c = 0; c < NF; ++c) r[c * NP + n] = fmaf(l, F[c], r[c * NP + n]);
+        }
       }
     }
   }

@@ -100,6 +100,16 @@ extern "C" int DG_CAT3(dgk_epk_upload_, DG_MODEL, DG_N)(const float *D, const fl
     if (fmask[i] != FM.v[i]) return -1;
   cudaError_t e = cudaMemcpyToSymbol(dgk::c_epk_D, D, sizeof(float) * 3 * Dg::NP * Dg::NP);
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_epk_L, L, sizeof(float) * Dg::NP * Dg::NFACE);
+  {   // the same operators with the output node fastest (FFMA2 operand pairs)
+    float Dt[3 * Dg::NP * Dg::NP], Lt[Dg::NFACE * Dg::NP];
+    for (int j = 0; j < 3; ++j)
+      for (int n = 0; n < Dg::NP; ++n)
+        for (int m = 0; m < Dg::NP; ++m) Dt[(j * Dg::NP + m) * Dg::NP + n] = D[(j * Dg::NP + n) * Dg::NP + m];
+    for (int n = 0; n < Dg::NP; ++n)
+      for (int j = 0; j < Dg::NFACE; ++j) Lt[j * Dg::NP + n] = L[n * Dg::NFACE + j];
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_epk_Dt, Dt, sizeof(Dt));
+    if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_epk_Lt, Lt, sizeof(Lt));
+  }
   if (e == cudaSuccess) e = cudaMemcpyToSymbol(dgk::c_epk_nbrnode, nbrnode, sizeof(unsigned short) * 4 * 24 * Dg::NFP);
   return (int)e;
 #else
