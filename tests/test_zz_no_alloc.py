@@ -38,6 +38,9 @@ def _case(model, N, n):
     (W.ELASTIC, 4, 5, {}, "tc_pipe"),
     (W.ACOUSTIC, 3, 5, {"variant": 1}, "simt_fused"),
     (W.ELASTIC, 3, 4, {"surface": 1}, "tc_pipe"),
+    (W.ACOUSTIC, 2, 1, {}, "simt_row_per_thread"),          # K = 6: less than one tile / one CTA
+    (W.ELASTIC, 1, 1, {}, "simt_elem_per_thread"),
+    (W.ELASTIC, 10, 2, {}, "tc_pipe"),                      # padded rows (Np = 286 -> 288), two CTAs per batch
 ])
 def test_step_static_matches_step_two_calls_in_a_row(dg, model, N, n, opts, kernel):
     case = Case(dg, _case(model, N, n), only_elems=np.arange(4), **opts)
